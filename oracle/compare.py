@@ -1,0 +1,154 @@
+"""Comparator: GPU results vs the oracle under BASELINE.json:north_star's tolerances.
+
+TEST INFRASTRUCTURE (same import rule as spd_oracle.py).  Pure numpy on arrays the caller
+hands in; the "GPU" side arrives as plain numpy arrays, nothing here imports the CUDA path.
+
+Rules (SURVEY.md §8(c) "Comparator"):
+  mu          |d| <= 1e-6 * max(|mu|, sigma)
+  sigma       |d| <= 1e-6 * sigma           (sigma_Nmax likewise)
+  SNR         every sample |d| <= max(1e-3, 1e-4 * |snr_oracle|)
+  width       equal wherever the oracle's margin (best - second best) > 1e-3; elsewhere the GPU's
+              width must be one whose oracle SNR (direct summation) is within 1e-3 of the best
+  candidates  equal as SETS of (dm, t) after dropping, from both sides, samples whose oracle SNR
+              is within 1e-3 of the threshold; matched records obey the SNR / width rules
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import Dict, Optional
+
+import numpy as np
+
+from . import spd_oracle as O
+
+SNR_ABS = 1e-3
+SNR_REL = 1e-4
+TIE = 1e-3
+STAT_REL = 1e-6
+
+
+@dataclass
+class Report:
+    ok: bool = True
+    msgs: list = field(default_factory=list)
+    info: Dict[str, float] = field(default_factory=dict)
+
+    def fail(self, m: str):
+        self.ok = False
+        self.msgs.append(m)
+
+    def __bool__(self):
+        return self.ok
+
+    def __str__(self):
+        return ("OK " if self.ok else "FAIL ") + "; ".join(self.msgs) + " " + str(self.info)
+
+
+def compare_stats(g_mean: float, g_sigma: float, o: O.Stats, g_sigma_nmax: Optional[float] = None) -> Report:
+    r = Report()
+    tol_mu = STAT_REL * max(abs(o.mean), o.sigma)
+    r.info["d_mean"] = abs(g_mean - o.mean)
+    r.info["d_sigma_rel"] = abs(g_sigma - o.sigma) / o.sigma
+    if not abs(g_mean - o.mean) <= tol_mu:
+        r.fail(f"mean {g_mean!r} vs {o.mean!r} (tol {tol_mu:.3g})")
+    if not abs(g_sigma - o.sigma) <= STAT_REL * o.sigma:
+        r.fail(f"sigma {g_sigma!r} vs {o.sigma!r}")
+    if g_sigma_nmax is not None:
+        r.info["d_sigma_nmax_rel"] = abs(g_sigma_nmax - o.sigma_nmax) / o.sigma_nmax
+        if not abs(g_sigma_nmax - o.sigma_nmax) <= STAT_REL * o.sigma_nmax:
+            r.fail(f"sigma_nmax {g_sigma_nmax!r} vs {o.sigma_nmax!r}")
+    return r
+
+
+def compare_planes(x: np.ndarray, mu: float, sig: np.ndarray,
+                   g_snr: np.ndarray, g_width: np.ndarray,
+                   o_snr: np.ndarray, o_width: np.ndarray, o_margin: np.ndarray,
+                   dm_offset_rows: Optional[np.ndarray] = None) -> Report:
+    """x is the float32 input the ORACLE planes were computed from (rows aligned with the planes)."""
+    r = Report()
+    g_snr = np.asarray(g_snr, dtype=np.float64)
+    g_width = np.asarray(g_width).astype(np.int64)
+    if g_snr.shape != o_snr.shape or g_width.shape != o_width.shape:
+        r.fail(f"shape {g_snr.shape}/{g_width.shape} vs {o_snr.shape}")
+        return r
+    if not np.all(np.isfinite(g_snr)):
+        r.fail(f"{np.count_nonzero(~np.isfinite(g_snr))} non-finite GPU SNR values")
+        return r
+    d = np.abs(g_snr - o_snr)
+    tol = np.maximum(SNR_ABS, SNR_REL * np.abs(o_snr))
+    bad = d > tol
+    r.info["snr_max_abs_err"] = float(d.max()) if d.size else 0.0
+    r.info["snr_violations"] = int(bad.sum())
+    if bad.any():
+        i = np.argwhere(bad)[0]
+        r.fail(f"SNR: {int(bad.sum())} samples out of tolerance, first at {tuple(i)}: "
+               f"{g_snr[tuple(i)]!r} vs {o_snr[tuple(i)]!r}")
+    mism = g_width != o_width
+    r.info["width_mismatch"] = int(mism.sum())
+    hard = mism & (o_margin > TIE)
+    if hard.any():
+        i = np.argwhere(hard)[0]
+        r.fail(f"width: {int(hard.sum())} mismatches outside near-ties, first at {tuple(i)}: "
+               f"{int(g_width[tuple(i)])} vs {int(o_width[tuple(i)])} (margin {o_margin[tuple(i)]:.3g})")
+    soft = mism & ~(o_margin > TIE)
+    r.info["width_near_tie_exempt"] = int(soft.sum())
+    r.info["near_tie_rate"] = float(np.count_nonzero(~(o_margin > TIE))) / max(1, o_margin.size)
+    if soft.any():
+        idx = np.argwhere(soft)
+        s_at = O.snr_at(x, mu, sig, idx[:, 0], idx[:, 1], g_width[soft].astype(np.int32))
+        best = o_snr[soft]
+        worse = ~(np.abs(s_at - best) <= TIE)   # NaN (width that does not fit) counts as a failure
+        if worse.any():
+            k = int(np.argmax(worse))
+            r.fail(f"width: {int(worse.sum())} near-tie widths whose oracle SNR is not within {TIE} of best, "
+                   f"first at {tuple(idx[k])}: width {int(g_width[soft][k])} snr {s_at[k]!r} vs best {best[k]!r}")
+    return r
+
+
+def compare_candidates(g_dm, g_t, g_snr, g_width, g_count: int, capacity: int,
+                       o_snr: np.ndarray, o_width: np.ndarray, o_margin: Optional[np.ndarray],
+                       f_T: float) -> Report:
+    """GPU list (unordered) vs the brute filter of the oracle planes, as sets of (dm, t)."""
+    r = Report()
+    n_dm, n_t = o_snr.shape
+    g_dm = np.asarray(g_dm).astype(np.int64); g_t = np.asarray(g_t).astype(np.int64)
+    g_snr = np.asarray(g_snr, dtype=np.float64); g_width = np.asarray(g_width).astype(np.int64)
+    if g_count > capacity:
+        r.fail(f"overflow: count {g_count} > capacity {capacity} (comparison needs the whole list)")
+        return r
+    if g_dm.size != g_count:
+        r.fail(f"list length {g_dm.size} != count {g_count}")
+        return r
+    if g_count and (g_dm.min() < 0 or g_dm.max() >= n_dm or g_t.min() < 0 or g_t.max() >= n_t):
+        r.fail("candidate index out of range")
+        return r
+    gkey = g_dm * n_t + g_t
+    if np.unique(gkey).size != gkey.size:
+        r.fail("duplicate (dm, t) records in the GPU list")
+    near = np.abs(o_snr - f_T) <= TIE
+    okey_all = np.flatnonzero((o_snr >= f_T).ravel())
+    near_flat = near.ravel()
+    okey = okey_all[~near_flat[okey_all]]
+    gkeep = ~near_flat[gkey]
+    r.info["oracle_hits"] = int(okey_all.size)
+    r.info["gpu_hits"] = int(g_count)
+    r.info["near_threshold_exempt"] = int(near.sum())
+    gk = np.sort(gkey[gkeep])
+    if gk.size != okey.size or not np.array_equal(gk, okey):
+        missing = np.setdiff1d(okey, gk); extra = np.setdiff1d(gk, okey)
+        r.fail(f"candidate sets differ: {missing.size} missing, {extra.size} extra "
+               f"(first missing {divmod(int(missing[0]), n_t) if missing.size else None}, "
+               f"first extra {divmod(int(extra[0]), n_t) if extra.size else None})")
+        return r
+    # matched records: SNR and width rules
+    os_ = o_snr.ravel()[gkey]; ow = o_width.ravel()[gkey]
+    d = np.abs(g_snr - os_)
+    bad = d > np.maximum(SNR_ABS, SNR_REL * np.abs(os_))
+    if bad.any():
+        r.fail(f"{int(bad.sum())} candidate SNRs out of tolerance")
+    wm = g_width != ow
+    if o_margin is not None:
+        wm &= o_margin.ravel()[gkey] > TIE
+    if wm.any():
+        r.fail(f"{int(wm.sum())} candidate widths differ outside near-ties")
+    return r

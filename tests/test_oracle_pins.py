@@ -1,0 +1,336 @@
+"""Pins P1-P9 of SURVEY.md §8(c): the oracle against what the paper and the mathematics fix.
+
+None of these retype the oracle's own formulae: they use numpy's two-pass mean/std, closed
+forms, brute-force inner sums written differently (O(n*Nmax^2)), invariances and statistics.
+A dropped term, wrong sign, shifted index or transposed operand in oracle/spd_oracle.c
+fails at least one of them.  CPU only.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import gen
+from oracle import spd_oracle as O
+
+
+def rng(seed):
+    return np.random.Generator(np.random.PCG64(seed))
+
+
+# ---------------------------------------------------------------- P1: eq.1/eq.2 == two-pass definition
+@pytest.mark.parametrize("shape,mu,sigma", [((1, 1), 0, 1), ((1, 2), 3, 1), ((1, 7), 0, 1), ((3, 333), 5, 2),
+                                             ((1, 1000), -7, 3), ((1, 1001), 100, 20), ((5, 4099), 100, 20),
+                                             ((64, 1000), 0, 1)])
+def test_p1_stats_equal_two_pass(shape, mu, sigma):
+    x = (mu + sigma * rng(1).standard_normal(shape)).astype(np.float32)
+    s = O.stats(x)
+    x64 = x.astype(np.float64)
+    assert s.n == x.size
+    assert s.mean == pytest.approx(x64.mean(), rel=1e-12, abs=1e-13)
+    assert s.sigma == pytest.approx(x64.std(ddof=0), rel=1e-12, abs=1e-13)
+    assert s.T == pytest.approx(x64.sum(), rel=1e-12, abs=1e-10)
+
+
+def test_p1_population_not_sample_sigma():
+    # reading A2: sigma = sqrt(S/j).  ddof=1 differs by 5e-4 relative at n=1000.
+    x = rng(2).standard_normal((1, 1000)).astype(np.float32)
+    s = O.stats(x)
+    assert abs(s.sigma - x.astype(np.float64).std(ddof=1)) / s.sigma > 1e-4
+    assert abs(s.sigma - x.astype(np.float64).std(ddof=0)) / s.sigma < 1e-12
+
+
+def test_p1_row_stride_is_respected():
+    big = rng(3).standard_normal((6, 50)).astype(np.float32)
+    view = big[:, :37]
+    s = O.stats(view)
+    assert s.n == 6 * 37
+    assert s.mean == pytest.approx(view.astype(np.float64).mean(), rel=1e-12)
+    assert s.sigma == pytest.approx(view.astype(np.float64).std(), rel=1e-12)
+
+
+def test_p1_block_size_does_not_matter():
+    x = (100 + 20 * rng(4).standard_normal((3, 2500))).astype(np.float32)
+    ref = O.stats(x, block=1000)
+    for b in (1, 2, 7, 999, 10**9):
+        s = O.stats(x, block=b)
+        assert s.mean == pytest.approx(ref.mean, rel=1e-13)
+        assert s.sigma == pytest.approx(ref.sigma, rel=1e-12)
+
+
+# ---------------------------------------------------------------- P2: closed forms
+def test_p2_constant():
+    s = O.stats(np.full((2, 777), 3.25, dtype=np.float32))
+    assert s.mean == 3.25 and s.sigma < 1e-12      # eq. 2's (n/m) T rounds: not exactly 0
+
+
+@pytest.mark.parametrize("n", [2, 10, 1000, 4097])
+def test_p2_ramp(n):
+    s = O.stats(np.arange(1, n + 1, dtype=np.float32).reshape(1, n))
+    assert s.mean == pytest.approx((n + 1) / 2, rel=1e-14)
+    assert s.sigma ** 2 == pytest.approx((n * n - 1) / 12, rel=1e-12)
+
+
+def test_p2_alternating():
+    x = np.tile(np.array([1, -1], dtype=np.float32), 3000).reshape(2, 3000)
+    s = O.stats(x)
+    assert s.mean == pytest.approx(0.0, abs=1e-15) and s.sigma == pytest.approx(1.0, rel=1e-14)
+
+
+def test_eq1_as_printed_without_square_is_wrong():
+    # reading A1: the S update needs the square.  S from the oracle matches sum((x-mean)^2); the
+    # unsquared printed form does not even have the right sign in general.
+    v = rng(5).standard_normal(1000) * 1.0
+    m, T, S = O.chan_run(v)
+    assert S == pytest.approx(((v - v.mean()) ** 2).sum(), rel=1e-12)
+    Tp, Sp = v[0], 0.0
+    for j in range(2, v.size + 1):
+        Tp += v[j - 1]
+        Sp += (j * v[j - 1] - Tp) / (j * (j - 1))
+    assert abs(Sp - S) / S > 0.5
+
+
+# ---------------------------------------------------------------- P3: eq.2 merge-order invariance
+def test_p3_merge_order_invariance():
+    g = rng(6)
+    v = 100 + 20 * g.standard_normal(10007)
+    cuts = np.sort(g.choice(np.arange(1, v.size), size=40, replace=False))
+    parts = [O.chan_run(p) for p in np.split(v, cuts)]
+    want_S = ((v - v.mean()) ** 2).sum()
+    # left fold
+    a = parts[0].copy()
+    for p in parts[1:]:
+        a = O.merge(a, p)
+    # random binary tree
+    pool = [p.copy() for p in parts]
+    while len(pool) > 1:
+        i = int(g.integers(0, len(pool) - 1))
+        pool[i:i + 2] = [O.merge(pool[i], pool[i + 1])]
+    # shuffled order (the sets are disjoint, the formula does not need adjacency)
+    perm = g.permutation(len(parts))
+    c = parts[perm[0]].copy()
+    for k in perm[1:]:
+        c = O.merge(c, parts[k])
+    for r in (a, pool[0], c):
+        assert r[0] == v.size
+        assert r[1] == pytest.approx(v.sum(), rel=1e-12)
+        assert r[2] == pytest.approx(want_S, rel=1e-12)
+
+
+def test_p3_merge_unequal_sizes_and_empty():
+    v = rng(7).standard_normal(50)
+    a, b = O.chan_run(v[:3]), O.chan_run(v[3:])
+    ab = O.merge(a, b)
+    assert ab[2] == pytest.approx(((v - v.mean()) ** 2).sum(), rel=1e-12)
+    e = np.zeros(3)
+    assert np.array_equal(O.merge(a, e), a)
+    assert np.array_equal(O.merge(e, a), a)
+
+
+# ---------------------------------------------------------------- O1b: sigma_Nmax
+@pytest.mark.parametrize("nmax", [1, 2, 5, 16])
+def test_sigma_nmax_brute(nmax):
+    x = (3 + rng(8).standard_normal((4, 100))).astype(np.float32)
+    s = O.sigma_nmax(x, nmax)
+    b = np.array([[x[d, t:t + nmax].astype(np.float64).sum() for t in range(100 - nmax + 1)] for d in range(4)])
+    assert s.n == b.size
+    assert s.mean == pytest.approx(b.mean(), rel=1e-12)
+    assert s.sigma == pytest.approx(b.std(), rel=1e-11)
+
+
+# ---------------------------------------------------------------- P8: sigma table
+def test_p8_sigma_table():
+    sigma, snm, nmax = 2.5, 40.0, 32
+    for mode in ("sqrt", "linear", "anchored"):
+        t = O.sigma_table(sigma, snm, nmax, mode)
+        assert t.shape == (nmax,)
+        assert t[0] == sigma                       # sigma_1 = sigma in every mode
+    t4 = O.sigma_table(sigma, snm, nmax, "sqrt")
+    assert np.allclose(t4, np.sqrt(np.arange(1, nmax + 1)) * sigma, rtol=1e-15)
+    t5 = O.sigma_table(sigma, snm, nmax, "linear")
+    assert t5[-1] == pytest.approx(math.sqrt(nmax) * sigma + snm, rel=1e-15)     # eq. 5 literal at N = Nmax
+    assert t5[16] == pytest.approx(math.sqrt(17) * sigma + 16 * snm / 31, rel=1e-15)
+    ta = O.sigma_table(sigma, snm, nmax, "anchored")
+    assert ta[-1] == pytest.approx(snm, rel=1e-14)
+    for mode in ("sqrt", "linear", "anchored"):      # Nmax = 1 drops the linear term
+        assert O.sigma_table(sigma, snm, 1, mode)[0] == sigma
+
+
+def test_p8_white_noise_sigma_nmax_close_to_eq4():
+    x = rng(9).standard_normal((8, 20000)).astype(np.float32)
+    s = O.full_stats(x, 32)
+    assert s.sigma_nmax == pytest.approx(math.sqrt(32) * s.sigma, rel=0.05)
+
+
+# ---------------------------------------------------------------- P4: rectangular pulse closed form (Figure 1)
+@pytest.mark.parametrize("W", [1, 2, 5, 16, 32])
+def test_p4_rect_pulse_closed_form(W):
+    nmax, n_t, p, A = 32, 400, 150, 3.0
+    x = np.zeros((1, n_t), dtype=np.float32)
+    x[0, p:p + W] = A
+    sig = O.sigma_table(1.0, float("nan"), nmax, "sqrt")
+    snr, width, _ = O.sweep(x, 0.0, sig)
+    # global maximum at (t = p, width = W), SNR = A sqrt(W): the best-fit boxcar wins
+    assert np.unravel_index(np.argmax(snr), snr.shape) == (0, p)
+    assert width[0, p] == W and snr[0, p] == pytest.approx(A * math.sqrt(W), rel=1e-14)
+    for k in range(0, nmax):                       # t = p - k
+        t = p - k
+        if W + k <= nmax:
+            assert width[0, t] == W + k, (k, width[0, t])
+            assert snr[0, t] == pytest.approx(A * W / math.sqrt(W + k), rel=1e-14)
+        else:
+            assert width[0, t] == nmax
+            assert snr[0, t] == pytest.approx(A * (nmax - k) / math.sqrt(nmax), rel=1e-14)
+    for j in range(0, W):                          # t = p + j inside the pulse
+        assert width[0, p + j] == W - j
+        assert snr[0, p + j] == pytest.approx(A * math.sqrt(W - j), rel=1e-14)
+    outside = np.ones(n_t, bool)
+    outside[p - nmax + 1:p + W] = False
+    assert np.all(snr[0, outside] == 0.0) and np.all(width[0, outside] == 1)
+
+
+# ---------------------------------------------------------------- P5: constant input: tie-break + row-end rule
+def test_p5_constant_and_zero():
+    nmax, n_t, c = 16, 100, 2.0
+    sig = O.sigma_table(1.0, float("nan"), nmax, "sqrt")
+    snr, width, margin = O.sweep(np.full((2, n_t), c, dtype=np.float32), 0.0, sig)
+    want_w = np.minimum(nmax, n_t - np.arange(n_t))
+    assert np.array_equal(width[0], want_w) and np.array_equal(width[1], want_w)   # only widths that fit (A9)
+    assert np.allclose(snr[0], c * np.sqrt(want_w), rtol=1e-14)
+    assert margin[0, -1] == np.inf                                               # single width evaluated
+    snr, width, margin = O.sweep(np.zeros((1, n_t), dtype=np.float32), 0.0, sig)
+    assert np.all(snr == 0.0) and np.all(width == 1)                              # strict '>' keeps smallest (A7)
+    assert np.all(margin[0, :-1] == 0.0)
+
+
+def test_p5_negative_constant_prefers_width_one():
+    sig = O.sigma_table(1.0, float("nan"), 8, "sqrt")
+    snr, width, _ = O.sweep(np.full((1, 50), -1.0, dtype=np.float32), 0.0, sig)
+    assert np.all(width == 1) and np.all(snr == -1.0)
+
+
+# ---------------------------------------------------------------- P6: brute-force inner sums, integer data => exact
+@pytest.mark.parametrize("n_t,nmax,mode", [(40, 8, "sqrt"), (33, 33, "sqrt"), (64, 17, "linear"), (9, 1, "sqrt")])
+def test_p6_brute_force(n_t, nmax, mode):
+    g = rng(10 + n_t)
+    x = g.integers(-5, 9, size=(3, n_t)).astype(np.float32)
+    mu, sigma, snm = 1.5, 2.0, 11.0
+    sig = O.sigma_table(sigma, snm, nmax, mode)
+    snr, width, margin = O.sweep(x, mu, sig)
+    for d in range(3):
+        for t in range(n_t):
+            vals = []
+            for N in range(1, min(nmax, n_t - t) + 1):
+                B = 0.0
+                for k in range(N):                 # explicit inner sum, not a running sum
+                    B += float(x[d, t + k])
+                if mode == "sqrt":
+                    sN = math.sqrt(N) * sigma
+                else:
+                    sN = math.sqrt(N) * sigma + ((N - 1) * snm / (nmax - 1) if nmax > 1 else 0.0)
+                vals.append((B - N * mu) / sN)
+            best = max(vals)
+            assert snr[d, t] == pytest.approx(best, rel=1e-14, abs=1e-14)
+            assert width[d, t] == 1 + vals.index(best)      # first (smallest) width attaining the max
+            rest = sorted(vals, reverse=True)
+            want_margin = rest[0] - rest[1] if len(rest) > 1 else np.inf
+            assert margin[d, t] == pytest.approx(want_margin, abs=1e-13)
+
+
+def test_snr_at_matches_sweep_trace():
+    x = rng(20).standard_normal((2, 200)).astype(np.float32)
+    sig = O.sigma_table(1.0, 0, 16, "sqrt")
+    snr, width, _ = O.sweep(x, 0.1, sig)
+    dm = np.array([0, 1, 1]); t = np.array([5, 100, 199]); w = width[dm, t]
+    assert np.allclose(O.snr_at(x, 0.1, sig, dm, t, w), snr[dm, t], rtol=1e-13)
+    assert np.isnan(O.snr_at(x, 0.1, sig, [0], [199], [2])[0])       # does not fit
+
+
+# ---------------------------------------------------------------- P7: pure noise normalisation
+def test_p7_nmax1_is_standardised_data():
+    x = (100 + 20 * rng(21).standard_normal((4, 5000))).astype(np.float32)
+    s = O.stats(x)
+    snr, width, _ = O.sweep(x, s.mean, O.sigma_table(s.sigma, 0, 1, "sqrt"))
+    assert np.all(width == 1)
+    assert np.allclose(snr, (x.astype(np.float64) - s.mean) / s.sigma, rtol=1e-13, atol=1e-13)
+    assert abs(snr.mean()) < 1e-12 and snr.std() == pytest.approx(1.0, rel=1e-12)
+
+
+@pytest.mark.parametrize("mu,sigma", [(0.0, 1.0), (100.0, 20.0)])
+@pytest.mark.parametrize("N", [1, 4, 64])
+def test_p7_fixed_width_planes_are_unit_normal(mu, sigma, N):
+    x = (mu + sigma * rng(22).standard_normal((4, 65536))).astype(np.float32)
+    s = O.stats(x)
+    pl = O.snr_fixed_width(x, s.mean, math.sqrt(N) * s.sigma, N)
+    v = pl[np.isfinite(pl)]
+    assert v.size == 4 * (65536 - N + 1)
+    assert abs(v.mean()) < 0.05 and v.std() == pytest.approx(1.0, abs=0.06)
+    # the form printed in Alg. 1, (B - mu)/sigma_N, would put the mean at (N-1) mu / (sqrt(N) sigma)  (reading A5)
+    if mu != 0 and N > 1:
+        assert abs((N - 1) * mu / (math.sqrt(N) * sigma)) > 1.0
+
+
+def test_max_plane_sanity_on_noise():
+    x = rng(23).standard_normal((8, 32768)).astype(np.float32)
+    snr, _, margin = O.sweep(x, 0.0, O.sigma_table(1.0, 0, 32, "sqrt"))
+    assert snr.mean() == pytest.approx(1.07, abs=0.05) and snr.std() == pytest.approx(0.84, abs=0.05)
+    assert 0.002 < np.mean(margin <= 1e-3) < 0.02       # near-tie rate on noise (~0.6 % at Nmax = 32)
+
+
+# ---------------------------------------------------------------- P9: candidates
+def test_p9_candidates_are_the_brute_filter_and_threshold_is_inclusive():
+    x = rng(24).integers(-2, 3, size=(4, 300)).astype(np.float32)
+    x[2, 100:104] = 5.0
+    sig = O.sigma_table(1.0, 0, 8, "sqrt")
+    snr, width, _ = O.sweep(x, 0.0, sig)
+    f_T = 10.0                                      # 4 * 5 / sqrt(4) = 10 exactly: '>=' keeps it
+    assert snr[2, 100] == 10.0
+    dm, t, s, w = O.candidates(snr, width, f_T)
+    keep = np.argwhere(snr >= f_T)
+    assert np.array_equal(np.stack([dm, t], 1), keep)
+    assert (2, 100) in set(zip(dm.tolist(), t.tolist()))
+    assert np.array_equal(s, snr[snr >= f_T]) and np.array_equal(w, width[snr >= f_T])
+    assert O.candidates(snr, width, np.nextafter(10.0, 11.0))[0].size < dm.size
+
+
+def test_p9_config1_recovers_every_injected_pulse():
+    cfg = gen.get_config(1)
+    x = gen.make_array(cfg)
+    res = O.search(x, cfg.nmax[0], cfg.sigma_mode, cfg.threshold)
+    dm, t, s, w = res["cand"]
+    for p in gen.pulse_table(cfg):
+        sel = (dm == p.row) & (np.abs(t - p.start) <= cfg.nmax[0])
+        assert sel.any(), p
+        k = np.argmax(np.where(sel, s, -np.inf))
+        assert abs(s[k] - p.snr) < 3.0, (p, s[k])
+        assert abs(int(t[k]) - p.start) <= max(2, p.width // 2)
+        assert 0.5 * p.width <= w[k] <= 2 * p.width + 1, (p, w[k])
+    # noise-only false alarms at 6 sigma over 1e6 samples x 32 widths must be rare
+    pulse_rows = {p.row for p in gen.pulse_table(cfg)}
+    assert sum(1 for d in dm.tolist() if d not in pulse_rows) <= 3
+
+
+def test_gaussian_profile_best_width_is_about_1p2_fwhm():
+    cfg = gen.custom_config(1, 4096, cid=1234, pulse_kind="none",
+                            extra_pulses=(gen.Pulse(0, 2000, 16, 5.0, float("nan"), "gauss"),))
+    x = gen.make_rows(cfg, [0]) * 0 + gen.make_rows(cfg, [0])   # noise included
+    clean = np.zeros_like(x)
+    t = np.arange(4096)
+    clean[0] = 5.0 * np.exp(-4 * math.log(2) * ((t - 2000) / 16.0) ** 2)
+    snr, width, _ = O.sweep(clean, 0.0, O.sigma_table(1.0, 0, 128, "sqrt"))
+    k = np.argmax(snr[0])
+    assert 1.0 * 16 <= width[0, k] <= 1.4 * 16
+    assert snr[0, k] == pytest.approx(5.0 * 0.8186 * math.sqrt(16), rel=0.02)
+
+
+def test_golden_rect_pulse():
+    """tests/golden/rect_pulse_W5_nmax32.txt: the P4 closed form tabulated by tests/golden/make_golden.py."""
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "rect_pulse_W5_nmax32.txt")
+    tab = np.loadtxt(path)
+    n_t = tab.shape[0]
+    x = np.zeros((1, n_t), dtype=np.float32)
+    x[0, 150:155] = 3.0
+    snr, width, _ = O.sweep(x, 0.0, O.sigma_table(1.0, 0, 32, "sqrt"))
+    assert np.array_equal(width[0], tab[:, 1].astype(np.int32))
+    assert np.allclose(snr[0], tab[:, 2], rtol=1e-14, atol=0)
