@@ -1,0 +1,125 @@
+/*
+ * spd.h -- C ABI of libspd: single-pulse detection on de-dispersed data, native to NVIDIA B200 (sm_100a).
+ *
+ * Method: K. Adamek & W. Armour, "A Real-time Single Pulse Detection Algorithm for GPUs",
+ * arXiv 1611.09704.  Citations are lines of /root/reference/PAPER.md ("PAPER.md:NN") plus section.
+ *
+ * Data: x is float32 [n_dm][n_t], row-major, time fastest ("de-dispersed time series data",
+ * PAPER.md:15; one row per DM trial).  row_stride is in ELEMENTS, >= n_t, and is shared
+ * by x and by the snr / width planes.
+ *
+ * Ownership: the caller owns every buffer, including the workspace; the library allocates nothing
+ * and keeps no state.  Unless a parameter is named h_*, every pointer is a DEVICE pointer.
+ * Asynchrony: every spd_* call that takes a stream only enqueues work on it and returns; it never
+ * synchronises (spd_search_host is the one exception, see there).
+ * Errors: return code only.  Argument checks -> SPD_ERR_INVALID_ARG; short workspace ->
+ * SPD_ERR_WORKSPACE; launch / runtime failure -> SPD_ERR_CUDA.  There is no CPU fallback.
+ * Undefined input: non-finite samples; sigma = 0.
+ */
+#ifndef SPD_H
+#define SPD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { SPD_OK = 0, SPD_ERR_INVALID_ARG = 1, SPD_ERR_CUDA = 2, SPD_ERR_WORKSPACE = 3 } spd_status;
+
+/* sigma after an N-sample boxcar (section 2.2) */
+typedef enum {
+    SPD_SIGMA_SQRT = 0,            /* eq. 4: sigma_N = sqrt(N) sigma */
+    SPD_SIGMA_LINEAR = 1,          /* eq. 5 exactly as printed: sqrt(N) sigma + (N-1) sigma_Nmax/(Nmax-1) */
+    SPD_SIGMA_LINEAR_ANCHORED = 2  /* not in the paper: sqrt(N) sigma + (N-1)(sigma_Nmax - sqrt(Nmax) sigma)/(Nmax-1) */
+} spd_sigma_mode;
+
+/* Result of spd_stats, in DEVICE memory (80 bytes).  (n, T, S) and (n_b, T_b, S_b) are the raw Chan
+ * triples so that several results can be merged with eq. 2 (spd_stats_merge).
+ * sigma_nmax = NaN, nmax_of_sigma = 0 when the sigma_Nmax pass was skipped. */
+typedef struct {
+    double   mean;           /* mu = T/n */
+    double   sigma;          /* sigma = sqrt(S/n), population form */
+    double   sigma_nmax;     /* std of the Nmax-sample boxcar SUMS over all full windows */
+    double   T, S;           /* sum, sum of squared deviations of the samples */
+    double   T_b, S_b;       /* the same for the boxcar sums */
+    uint64_t n;              /* number of samples */
+    uint64_t n_b;            /* number of boxcar sums: n_dm * (n_t - nmax + 1) */
+    int32_t  nmax_of_sigma;  /* the Nmax sigma_nmax was measured for */
+    int32_t  _pad;
+} spd_stats_t;
+
+/* One detection ("dispersion measure (DM) and the time at which an event was detected,
+ * its SNR and the width of the boxcar responsible").  dm = row index, t = index of the FIRST sample of
+ * the best boxcar; physical DM and time are a caller-side affine map.  16 bytes, one 128-bit store. */
+typedef struct { uint32_t dm, t; float snr; uint32_t width; } spd_candidate_t;
+
+const char *spd_status_string(spd_status s);
+
+/* Bytes of device workspace spd_stats / spd_boxcar_snr need for this shape (the larger of the two).
+ * Returns 0 for invalid arguments. */
+size_t spd_workspace_bytes(int64_t n_dm, int64_t n_t, int nmax);
+
+/* Step 1 -- mean and standard deviation (section 2.1).
+ * Kernel 1 cuts the array into equal blocks; each thread runs the streaming update eq. 1 over a fixed
+ * run and partial (n,T,S) are merged with eq. 2 inside the block; kernel 2 merges the block partials
+ * with eq. 2 in a fixed order (bit-reproducible) and writes *d_stats.
+ * nmax_for_sigma > 0 also measures the "true" sigma_Nmax that eq. 5 needs; 0 skips it.
+ * Requires 1 <= n_dm, 1 <= n_t, row_stride >= n_t, 0 <= nmax_for_sigma <= min(n_t, 4096).
+ * d_ws: workspace of >= spd_workspace_bytes() bytes, 16-byte aligned; contents need not persist. */
+spd_status spd_stats(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                     int nmax_for_sigma, spd_stats_t *d_stats,
+                     void *d_ws, size_t ws_bytes, void *stream);
+
+/* eq. 2 over `count` results of spd_stats on disjoint row blocks, folded in index
+ * order into *d_out (mean / sigma / sigma_nmax recomputed).  This is the one exchange step of a
+ * DM-row-sharded run: all-gather the 80-byte structs, then merge locally in rank order.
+ * d_parts and d_out are device pointers; d_out may alias d_parts[0]. */
+spd_status spd_stats_merge(const spd_stats_t *d_parts, int count, spd_stats_t *d_out, void *stream);
+
+/* Steps 2-4a -- boxcars of every width 1..nmax, SNR, max and arg-max over width, in one kernel
+ * (section 2.3, Algorithm 1 as read in DESIGN.md):
+ *   B_N(t) = sum_{k<N} x[d][t+k],  SNR_N(t) = (B_N(t) - N mu) / sigma_N,  widths with t+N <= n_t only;
+ *   d_snr[d][t] = max_N SNR_N(t),  d_width[d][t] = the smallest N attaining it.
+ * mu, sigma (and sigma_nmax for the LINEAR modes) are read from *d_stats on the device; a LINEAR mode
+ * fed stats whose nmax_of_sigma != nmax yields an all-NaN SNR plane (it cannot be caught without a sync).
+ * Requires 1 <= nmax <= min(n_t, 4096) (shared-memory bound of the tile).  d_width may be NULL (plane not written). */
+spd_status spd_boxcar_snr(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                          const spd_stats_t *d_stats, int nmax, spd_sigma_mode mode,
+                          float *d_snr, uint16_t *d_width,
+                          void *d_ws, size_t ws_bytes, void *stream);
+
+/* Step 4b -- candidate selection (section 2.4): every (d,t) with d_snr[d][t] >= threshold
+ * becomes one record; the planes are not modified; the list is unordered.
+ * *d_count is zeroed by the call and counts ALL hits; only the first `capacity` reservations are written,
+ * so the caller detects overflow as *d_count > capacity after its own synchronisation. */
+spd_status spd_candidates(const float *d_snr, const uint16_t *d_width, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                          float threshold, spd_candidate_t *d_out, uint64_t capacity,
+                          unsigned long long *d_count, void *stream);
+
+/* Steps 2-4 fused: the sweep of spd_boxcar_snr with the threshold of spd_candidates applied in the
+ * same kernel; the SNR / width planes are never written (the list is the only downstream product,
+ * PAPER.md:93).  Same records as spd_boxcar_snr + spd_candidates. */
+spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                            const spd_stats_t *d_stats, int nmax, spd_sigma_mode mode, float threshold,
+                            spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,
+                            void *d_ws, size_t ws_bytes, void *stream);
+
+/* Device bytes spd_search_host needs in d_arena for this shape and capacity. */
+size_t spd_search_host_arena_bytes(int64_t n_dm, int64_t n_t, int nmax, uint64_t capacity);
+
+/* The whole path from HOST buffers: copies h_x (row_stride = n_t) to the device, runs spd_stats,
+ * spd_boxcar_snr and spd_candidates, and copies the statistics, the hit count and the first
+ * min(count, capacity) records back.  h_x / h_out / h_count / h_stats are HOST pointers (pinned memory
+ * makes the copies asynchronous); d_arena is a caller-owned DEVICE buffer of >=
+ * spd_search_host_arena_bytes().  This call SYNCHRONISES `stream` before it returns. */
+spd_status spd_search_host(const float *h_x, int64_t n_dm, int64_t n_t, int nmax, spd_sigma_mode mode,
+                           float threshold, spd_candidate_t *h_out, uint64_t capacity,
+                           unsigned long long *h_count, spd_stats_t *h_stats,
+                           void *d_arena, size_t arena_bytes, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPD_H */

@@ -1,0 +1,12 @@
+"""spd-b200: single-pulse detection (arXiv 1611.09704) as hand-written sm_100a CUDA kernels behind a C ABI.
+
+`binding` is a thin ctypes layer over libspd.so (include/spd.h); `build` compiles the library in-tree.
+Nothing here computes on the CPU and nothing here imports the oracle.
+"""
+from .binding import (  # noqa: F401
+    SpdError, lib, LIB_PATH, STATS_DTYPE, CAND_DTYPE,
+    SPD_SIGMA_SQRT, SPD_SIGMA_LINEAR, SPD_SIGMA_LINEAR_ANCHORED,
+    workspace_bytes, new_workspace, new_stats, read_stats, write_stats, new_candidates, read_candidates,
+    spd_stats, spd_stats_merge, spd_boxcar_snr, spd_candidates, spd_search_fused,
+    search_host_arena_bytes, spd_search_host,
+)

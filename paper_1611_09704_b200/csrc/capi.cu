@@ -1,0 +1,155 @@
+// capi.cu -- the C ABI of include/spd.h: argument checks and launches only; every step runs in the kernels.
+#include "spd_common.cuh"
+
+using namespace spd;
+
+namespace {
+
+constexpr int NMAX_API_LIMIT = 4096;     // shared-memory bound of the sweep / sigma_Nmax tiles
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+inline bool shape_ok(int64_t n_dm, int64_t n_t, int64_t row_stride)
+{
+    return n_dm >= 1 && n_t >= 1 && row_stride >= n_t && n_dm <= 0xffffffffLL && n_t <= 0xffffffffLL;
+}
+inline bool nmax_ok(int nmax, int64_t n_t) { return nmax >= 1 && nmax <= NMAX_API_LIMIT && (int64_t)nmax <= n_t; }
+
+}  // namespace
+
+extern "C" {
+
+const char *spd_status_string(spd_status s)
+{
+    switch (s) {
+    case SPD_OK: return "SPD_OK";
+    case SPD_ERR_INVALID_ARG: return "SPD_ERR_INVALID_ARG";
+    case SPD_ERR_CUDA: return "SPD_ERR_CUDA";
+    case SPD_ERR_WORKSPACE: return "SPD_ERR_WORKSPACE";
+    }
+    return "SPD_ERR_UNKNOWN";
+}
+
+size_t spd_workspace_bytes(int64_t n_dm, int64_t n_t, int nmax)
+{
+    if (n_dm < 1 || n_t < 1 || nmax < 0 || nmax > NMAX_API_LIMIT) return 0;
+    size_t tab = sweep_table_bytes(nmax > 0 ? nmax : 1);
+    return align_up(STATS_WS > tab ? STATS_WS : tab, 256);
+}
+
+spd_status spd_stats(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
+                     spd_stats_t *d_stats, void *d_ws, size_t ws_bytes, void *stream)
+{
+    if (!d_x || !d_stats || !d_ws || !shape_ok(n_dm, n_t, row_stride)) return SPD_ERR_INVALID_ARG;
+    if (nmax_for_sigma < 0 || (nmax_for_sigma > 0 && !nmax_ok(nmax_for_sigma, n_t))) return SPD_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_ws) & 15) != 0) return SPD_ERR_INVALID_ARG;
+    if (ws_bytes < STATS_WS) return SPD_ERR_WORKSPACE;
+    cudaError_t e = launch_stats(d_x, n_dm, n_t, row_stride, nmax_for_sigma, d_stats, d_ws, (cudaStream_t)stream);
+    return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
+}
+
+spd_status spd_stats_merge(const spd_stats_t *d_parts, int count, spd_stats_t *d_out, void *stream)
+{
+    if (!d_parts || !d_out || count < 1) return SPD_ERR_INVALID_ARG;
+    cudaError_t e = launch_stats_merge(d_parts, count, d_out, (cudaStream_t)stream);
+    return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
+}
+
+spd_status spd_boxcar_snr(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                          const spd_stats_t *d_stats, int nmax, spd_sigma_mode mode,
+                          float *d_snr, uint16_t *d_width, void *d_ws, size_t ws_bytes, void *stream)
+{
+    if (!d_x || !d_stats || !d_snr || !d_ws || !shape_ok(n_dm, n_t, row_stride) || !nmax_ok(nmax, n_t))
+        return SPD_ERR_INVALID_ARG;
+    if ((int)mode < 0 || (int)mode > 2 || (reinterpret_cast<uintptr_t>(d_ws) & 15) != 0) return SPD_ERR_INVALID_ARG;
+    if (ws_bytes < sweep_table_bytes(nmax)) return SPD_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    float *table = reinterpret_cast<float *>(d_ws);
+    cudaError_t e = launch_sigma_table(d_stats, nmax, (int)mode, table, s);
+    if (e != cudaSuccess) return SPD_ERR_CUDA;
+    e = launch_sweep(d_x, n_dm, n_t, row_stride, d_stats, table, nmax, d_snr, d_width, false, 0.0f, nullptr, 0, nullptr, s);
+    return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
+}
+
+spd_status spd_candidates(const float *d_snr, const uint16_t *d_width, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                          float threshold, spd_candidate_t *d_out, uint64_t capacity,
+                          unsigned long long *d_count, void *stream)
+{
+    if (!d_snr || !d_width || !d_count || (!d_out && capacity > 0) || !shape_ok(n_dm, n_t, row_stride))
+        return SPD_ERR_INVALID_ARG;
+    if (threshold != threshold) return SPD_ERR_INVALID_ARG;
+    cudaError_t e = launch_candidates(d_snr, d_width, n_dm, n_t, row_stride, threshold, d_out, capacity, d_count,
+                                      (cudaStream_t)stream);
+    return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
+}
+
+spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                            const spd_stats_t *d_stats, int nmax, spd_sigma_mode mode, float threshold,
+                            spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,
+                            void *d_ws, size_t ws_bytes, void *stream)
+{
+    if (!d_x || !d_stats || !d_count || (!d_out && capacity > 0) || !d_ws || !shape_ok(n_dm, n_t, row_stride) ||
+        !nmax_ok(nmax, n_t))
+        return SPD_ERR_INVALID_ARG;
+    if ((int)mode < 0 || (int)mode > 2 || threshold != threshold || (reinterpret_cast<uintptr_t>(d_ws) & 15) != 0)
+        return SPD_ERR_INVALID_ARG;
+    if (ws_bytes < sweep_table_bytes(nmax)) return SPD_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    float *table = reinterpret_cast<float *>(d_ws);
+    if (cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s) != cudaSuccess) return SPD_ERR_CUDA;
+    cudaError_t e = launch_sigma_table(d_stats, nmax, (int)mode, table, s);
+    if (e != cudaSuccess) return SPD_ERR_CUDA;
+    e = launch_sweep(d_x, n_dm, n_t, row_stride, d_stats, table, nmax, nullptr, nullptr, true, threshold, d_out,
+                     capacity, d_count, s);
+    return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
+}
+
+// arena layout of spd_search_host: x | snr | width | candidates | stats | count | workspace
+size_t spd_search_host_arena_bytes(int64_t n_dm, int64_t n_t, int nmax, uint64_t capacity)
+{
+    if (n_dm < 1 || n_t < 1 || nmax < 1 || nmax > NMAX_API_LIMIT) return 0;
+    const size_t n = (size_t)n_dm * (size_t)n_t;
+    return align_up(n * 4, 256) + align_up(n * 4, 256) + align_up(n * 2, 256) +
+           align_up((size_t)capacity * sizeof(spd_candidate_t), 256) + 256 + 256 + spd_workspace_bytes(n_dm, n_t, nmax);
+}
+
+spd_status spd_search_host(const float *h_x, int64_t n_dm, int64_t n_t, int nmax, spd_sigma_mode mode,
+                           float threshold, spd_candidate_t *h_out, uint64_t capacity,
+                           unsigned long long *h_count, spd_stats_t *h_stats,
+                           void *d_arena, size_t arena_bytes, void *stream)
+{
+    if (!h_x || !h_count || (!h_out && capacity > 0) || !d_arena || !shape_ok(n_dm, n_t, n_t) || !nmax_ok(nmax, n_t))
+        return SPD_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_arena) & 255) != 0) return SPD_ERR_INVALID_ARG;
+    if (arena_bytes < spd_search_host_arena_bytes(n_dm, n_t, nmax, capacity)) return SPD_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t n = (size_t)n_dm * (size_t)n_t;
+    unsigned char *p = reinterpret_cast<unsigned char *>(d_arena);
+    float *d_x = reinterpret_cast<float *>(p);                 p += align_up(n * 4, 256);
+    float *d_snr = reinterpret_cast<float *>(p);               p += align_up(n * 4, 256);
+    uint16_t *d_width = reinterpret_cast<uint16_t *>(p);       p += align_up(n * 2, 256);
+    spd_candidate_t *d_out = reinterpret_cast<spd_candidate_t *>(p); p += align_up((size_t)capacity * sizeof(spd_candidate_t), 256);
+    spd_stats_t *d_stats = reinterpret_cast<spd_stats_t *>(p); p += 256;
+    unsigned long long *d_count = reinterpret_cast<unsigned long long *>(p); p += 256;
+    void *d_ws = p;
+    const size_t ws_bytes = spd_workspace_bytes(n_dm, n_t, nmax);
+
+    if (cudaMemcpyAsync(d_x, h_x, n * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPD_ERR_CUDA;
+    spd_status st = spd_stats(d_x, n_dm, n_t, n_t, mode == SPD_SIGMA_SQRT ? 0 : nmax, d_stats, d_ws, ws_bytes, stream);
+    if (st != SPD_OK) return st;
+    st = spd_boxcar_snr(d_x, n_dm, n_t, n_t, d_stats, nmax, mode, d_snr, d_width, d_ws, ws_bytes, stream);
+    if (st != SPD_OK) return st;
+    st = spd_candidates(d_snr, d_width, n_dm, n_t, n_t, threshold, d_out, capacity, d_count, stream);
+    if (st != SPD_OK) return st;
+    if (h_stats && cudaMemcpyAsync(h_stats, d_stats, sizeof(spd_stats_t), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
+    if (cudaMemcpyAsync(h_count, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
+    if (cudaStreamSynchronize(s) != cudaSuccess) return SPD_ERR_CUDA;
+    const unsigned long long got = *h_count < capacity ? *h_count : capacity;
+    if (got > 0) {
+        if (cudaMemcpyAsync(h_out, d_out, (size_t)got * sizeof(spd_candidate_t), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
+        if (cudaStreamSynchronize(s) != cudaSuccess) return SPD_ERR_CUDA;
+    }
+    return SPD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,333 @@
+"""-m gpu parity tests: the CUDA path (through the C-ABI binding) against the oracle, element by element.
+
+Tolerances are BASELINE.json:north_star's, implemented in oracle/compare.py:
+  mu |d| <= 1e-6 max(|mu|, sigma); sigma 1e-6 relative; SNR max(1e-3, 1e-4 |snr|); width exact outside
+  near-ties (margin <= 1e-3); candidates equal as (dm, t) sets outside 1e-3 of the threshold.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import gen
+from oracle import spd_oracle as O
+from oracle import compare as CMP
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1611_09704_b200 as P
+    P.lib()      # fails loudly when libspd.so is missing
+    return P
+
+
+def rng(seed):
+    return np.random.Generator(np.random.PCG64(seed))
+
+
+# ------------------------------------------------------------------------------------------- spd_stats
+@pytest.mark.parametrize("shape,mu,sigma,stride", [
+    ((1, 1), 3.0, 1.0, None), ((1, 5), 0.0, 1.0, None), ((3, 333), 5.0, 2.0, None), ((1, 4096), 0.0, 1.0, None),
+    ((1, 4097), 100.0, 20.0, None), ((7, 5000), 100.0, 20.0, None), ((64, 16384), 0.0, 1.0, None),
+    ((5, 4099), -1000.0, 1.0, None), ((6, 8192), 100.0, 20.0, 8200), ((6, 1000), 0.0, 1.0, 1003),
+    ((300, 70), 2.0, 3.0, None),
+])
+def test_stats_parity(P, shape, mu, sigma, stride):
+    from gpu_util import gpu_stats
+    x = (mu + sigma * rng(100).standard_normal(shape)).astype(np.float32)
+    g, _ = gpu_stats(x, 0, stride)
+    o = O.stats(x)
+    assert int(g["n"]) == x.size
+    if x.size == 1:
+        assert g["mean"] == float(x[0, 0]) and g["sigma"] == 0.0
+        return
+    r = CMP.compare_stats(float(g["mean"]), float(g["sigma"]), o)
+    assert r, str(r)
+    assert math.isnan(float(g["sigma_nmax"])) and int(g["nmax_of_sigma"]) == 0
+
+
+@pytest.mark.parametrize("shape,nmax", [((4, 100), 1), ((4, 100), 16), ((3, 5000), 512), ((2, 9000), 100), ((1, 64), 64),
+                                        ((9, 4200), 33)])
+def test_sigma_nmax_parity(P, shape, nmax):
+    from gpu_util import gpu_stats
+    x = (1.0 + rng(101).standard_normal(shape)).astype(np.float32)
+    x[0, 10:10 + min(40, shape[1] - 10)] += 6.0
+    g, _ = gpu_stats(x, nmax)
+    o = O.full_stats(x, nmax)
+    assert int(g["n_b"]) == shape[0] * (shape[1] - nmax + 1) and int(g["nmax_of_sigma"]) == nmax
+    if int(g["n_b"]) == shape[0]:                      # one window per row: sigma may be tiny but defined
+        assert float(g["sigma_nmax"]) == pytest.approx(o.sigma_nmax, rel=1e-6, abs=1e-9)
+    else:
+        r = CMP.compare_stats(float(g["mean"]), float(g["sigma"]), o, float(g["sigma_nmax"]))
+        assert r, str(r)
+
+
+def test_stats_is_bit_reproducible(P):
+    from gpu_util import gpu_stats
+    x = (100 + 20 * rng(102).standard_normal((64, 16384))).astype(np.float32)
+    a, _ = gpu_stats(x, 32)
+    b, _ = gpu_stats(x, 32)
+    assert a.tobytes() == b.tobytes()
+
+
+def test_stats_merge_equals_whole(P):
+    from gpu_util import to_dev
+    x = (100 + 20 * rng(103).standard_normal((10, 6000))).astype(np.float32)
+    parts = P.new_stats(count=3)
+    nb = P.STATS_DTYPE.itemsize
+    for i, (lo, hi) in enumerate([(0, 3), (3, 4), (4, 10)]):
+        P.spd_stats(to_dev(x[lo:hi]), 16, stats=parts[i * nb:(i + 1) * nb])
+    m = P.read_stats(P.spd_stats_merge(parts, 3))[0]
+    o = O.full_stats(x, 16)
+    assert int(m["n"]) == x.size and int(m["n_b"]) == 10 * (6000 - 15)
+    r = CMP.compare_stats(float(m["mean"]), float(m["sigma"]), o, float(m["sigma_nmax"]))
+    assert r, str(r)
+
+
+# ------------------------------------------------------------------------------------------- spd_boxcar_snr
+def _sweep_case(P, x, nmax, mode="sqrt", stats=None, stride=None, want_rate=None):
+    """Same (mu, sigma) on both sides: isolates the sweep kernel."""
+    from gpu_util import gpu_sweep
+    if stats is None:
+        o = O.full_stats(x, nmax if mode != "sqrt" else 0)
+    else:
+        o = stats
+    st = P.write_stats(o.mean, o.sigma, o.sigma_nmax, o.nmax_of_sigma)
+    sig = O.sigma_table(o.sigma, o.sigma_nmax, nmax, mode)
+    o_snr, o_w, o_m = O.sweep(x, o.mean, sig)
+    g_snr, g_w, dev = gpu_sweep(x, st, nmax, mode, stride)
+    r = CMP.compare_planes(x, o.mean, sig, g_snr, g_w, o_snr, o_w, o_m)
+    assert r, str(r)
+    return r, (o_snr, o_w, o_m), dev
+
+
+UNIT = O.Stats(0, 0.0, 0.0, 0.0, 1.0)
+
+
+@pytest.mark.parametrize("n_dm,n_t,nmax", [
+    (1, 1, 1), (1, 7, 1), (1, 7, 7), (3, 100, 8), (2, 100, 5), (2, 100, 13), (1, 1023, 16), (1, 1024, 32),
+    (1, 1025, 32), (2, 2047, 24), (2, 2048, 64), (3, 2049, 100), (2, 5000, 128), (1, 4097, 7), (5, 3000, 512),
+    (2, 600, 600), (1, 9001, 1000),
+])
+def test_sweep_integer_data_forced_stats(P, n_dm, n_t, nmax):
+    # small integers: every running sum is exact in fp32 and fp64 (pin P6 on the GPU side)
+    x = rng(200 + n_t).integers(-4, 6, size=(n_dm, n_t)).astype(np.float32)
+    _sweep_case(P, x, nmax, "sqrt", UNIT)
+
+
+@pytest.mark.parametrize("n_dm,n_t,nmax,mu,sigma", [
+    (4, 4096, 32, 0.0, 1.0), (3, 6000, 128, 0.0, 1.0), (3, 5000, 64, 100.0, 20.0), (2, 7777, 512, 0.0, 1.0),
+    (2, 4100, 100, -1000.0, 1.0), (64, 2048, 8, 0.0, 1.0),
+])
+def test_sweep_noise(P, n_dm, n_t, nmax, mu, sigma):
+    x = (mu + sigma * rng(300 + nmax).standard_normal((n_dm, n_t))).astype(np.float32)
+    r, _, _ = _sweep_case(P, x, nmax)
+    assert r.info["near_tie_rate"] < 0.05          # far above the expected 0.3-2 % would be a bug, not a tie
+
+
+@pytest.mark.parametrize("stride", [8200, 8196, 8193])
+def test_sweep_padded_row_stride(P, stride):
+    x = rng(310).standard_normal((3, 8192)).astype(np.float32)
+    _sweep_case(P, x, 32, stride=stride)
+
+
+def test_sweep_rect_pulse_closed_form_across_tile_edges(P):
+    # Figure-1 property on the GPU side: pulses straddling the sub-tile (1024), tile (2048) edges and the row end
+    from gpu_util import gpu_sweep
+    nmax, n_t, A = 32, 6144, 3.0
+    for p, W in [(1020, 8), (2040, 16), (2047, 1), (2048, 5), (4090, 32), (n_t - 5, 5), (n_t - 1, 1), (0, 3)]:
+        x = np.zeros((1, n_t), dtype=np.float32)
+        x[0, p:p + W] = A
+        g_snr, g_w, _ = gpu_sweep(x, P.write_stats(0.0, 1.0), nmax)
+        assert g_w[0, p] == W and g_snr[0, p] == pytest.approx(A * math.sqrt(W), rel=2e-7)
+        assert int(np.argmax(g_snr[0])) == p
+        for k in range(0, min(nmax, p + 1)):
+            if W + k <= nmax:
+                assert g_w[0, p - k] == W + k
+                assert g_snr[0, p - k] == pytest.approx(A * W / math.sqrt(W + k), rel=3e-7)
+
+
+def test_sweep_constant_input_tie_break_and_row_end(P):
+    from gpu_util import gpu_sweep
+    nmax, n_t = 16, 3000
+    g_snr, g_w, _ = gpu_sweep(np.full((2, n_t), 2.0, dtype=np.float32), P.write_stats(0.0, 1.0), nmax)
+    want = np.minimum(nmax, n_t - np.arange(n_t))
+    assert np.array_equal(g_w[0], want) and np.array_equal(g_w[1], want)
+    assert np.allclose(g_snr[0], 2.0 * np.sqrt(want), rtol=3e-7)
+    g_snr, g_w, _ = gpu_sweep(np.zeros((1, n_t), dtype=np.float32), P.write_stats(0.0, 1.0), nmax)
+    assert np.all(g_snr == 0.0) and np.all(g_w == 1)
+    g_snr, g_w, _ = gpu_sweep(np.full((1, n_t), -1.0, dtype=np.float32), P.write_stats(0.0, 1.0), nmax)
+    assert np.all(g_w == 1) and np.all(g_snr == -1.0)
+
+
+def test_sweep_nmax1_is_standardised_data(P):
+    from gpu_util import gpu_sweep
+    x = (100 + 20 * rng(320).standard_normal((4, 5000))).astype(np.float32)
+    o = O.stats(x)
+    g_snr, g_w, _ = gpu_sweep(x, P.write_stats(o.mean, o.sigma), 1)
+    assert np.all(g_w == 1)
+    assert np.allclose(g_snr, (x.astype(np.float64) - o.mean) / o.sigma, rtol=0, atol=2e-6)
+
+
+@pytest.mark.parametrize("mode", ["linear", "anchored"])
+def test_sweep_eq5_modes(P, mode):
+    x = rng(330).standard_normal((3, 6000)).astype(np.float32)
+    x[1, 1000:1300] += 5.0
+    _sweep_case(P, x, 512, mode)
+    _sweep_case(P, x, 100, mode)
+
+
+def test_sweep_linear_with_wrong_nmax_is_all_nan(P):
+    from gpu_util import gpu_sweep
+    x = rng(331).standard_normal((1, 3000)).astype(np.float32)
+    st = P.write_stats(0.0, 1.0, 10.0, 64)
+    g_snr, _, _ = gpu_sweep(x, st, 32, "linear")
+    assert np.all(np.isnan(g_snr))
+
+
+def test_sweep_without_width_plane(P):
+    from gpu_util import gpu_sweep
+    x = rng(332).standard_normal((2, 4096)).astype(np.float32)
+    a, w, _ = gpu_sweep(x, P.write_stats(0.0, 1.0), 32)
+    b, none, _ = gpu_sweep(x, P.write_stats(0.0, 1.0), 32, want_width=False)
+    assert none is None and np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------------------------------- spd_candidates / fused
+def test_candidates_threshold_inclusive_and_set_equality(P):
+    from gpu_util import gpu_sweep, gpu_candidates, gpu_fused
+    x = rng(400).integers(-2, 3, size=(4, 5000)).astype(np.float32)
+    x[2, 100:104] = 5.0                               # 4*5/sqrt(4) = 10 exactly
+    x[3, 4996:5000] = 5.0                             # at the row end
+    st = P.write_stats(0.0, 1.0)
+    sig = O.sigma_table(1.0, 0, 8, "sqrt")
+    o_snr, o_w, o_m = O.sweep(x, 0.0, sig)
+    g_snr, g_w, (d, s, w) = gpu_sweep(x, st, 8)
+    assert g_snr[2, 100] == 10.0
+    for thr in (10.0, 6.0, 3.0):
+        rec, total = gpu_candidates(s, w, thr)
+        assert total == int((g_snr >= np.float32(thr)).sum())
+        r = CMP.compare_candidates(rec["dm"], rec["t"], rec["snr"], rec["width"], total, 1 << 16, o_snr, o_w, o_m, thr)
+        assert r, str(r)
+        rec2, total2 = gpu_fused(d, st, 8, "sqrt", thr)
+        assert total2 == total
+        a = np.sort(rec, order=["dm", "t"]); b = np.sort(rec2, order=["dm", "t"])
+        assert a.tobytes() == b.tobytes()
+    rec, total = gpu_candidates(s, w, 10.0)
+    assert (2, 100) in set(zip(rec["dm"].tolist(), rec["t"].tolist()))       # '>=' keeps it
+    rec, total = gpu_candidates(s, w, float(np.nextafter(np.float32(10.0), np.float32(11.0))))
+    assert (2, 100) not in set(zip(rec["dm"].tolist(), rec["t"].tolist()))
+
+
+def test_candidates_overflow_convention(P):
+    from gpu_util import gpu_sweep, gpu_candidates
+    x = rng(401).standard_normal((8, 4096)).astype(np.float32)
+    g_snr, g_w, (d, s, w) = gpu_sweep(x, P.write_stats(0.0, 1.0), 16)
+    want = int((g_snr >= np.float32(1.0)).sum())
+    rec, total = gpu_candidates(s, w, 1.0, capacity=100)
+    assert total == want and total > 100 and rec.size == 100
+    assert np.all(g_snr[rec["dm"], rec["t"]] == rec["snr"]) and np.all(g_w[rec["dm"], rec["t"]] == rec["width"])
+    rec, total = gpu_candidates(s, w, 1e9)
+    assert total == 0 and rec.size == 0
+
+
+def test_candidates_ragged_and_strided(P):
+    from gpu_util import gpu_sweep, gpu_candidates
+    x = rng(402).standard_normal((5, 4101)).astype(np.float32)
+    g_snr, g_w, (d, s, w) = gpu_sweep(x, P.write_stats(0.0, 1.0), 16, row_stride=4104)
+    rec, total = gpu_candidates(s, w, 2.5)
+    keep = np.argwhere(g_snr >= np.float32(2.5))
+    got = np.stack([rec["dm"], rec["t"]], 1).astype(np.int64)
+    assert total == keep.shape[0]
+    assert np.array_equal(got[np.lexsort((got[:, 1], got[:, 0]))], keep)
+
+
+# ------------------------------------------------------------------------------------------- whole path
+def _whole_path(P, cfg, x, nmax, rows=None, fused=True):
+    """stats -> sweep -> candidates on the GPU; oracle on all rows, or on `rows` with the ORACLE's full-array stats."""
+    from gpu_util import gpu_candidates, gpu_fused
+    d = torch.from_numpy(x).cuda()
+    mode = cfg.sigma_mode
+    st = P.spd_stats(d, nmax if mode != "sqrt" else 0)
+    snr, width = P.spd_boxcar_snr(d, st, nmax, mode)
+    rec, total = gpu_candidates(snr, width, cfg.threshold, capacity=1 << 22)
+    g = P.read_stats(st)[0]
+    o = O.full_stats(x, nmax if mode != "sqrt" else 0)
+    r = CMP.compare_stats(float(g["mean"]), float(g["sigma"]), o, float(g["sigma_nmax"]) if mode != "sqrt" else None)
+    assert r, str(r)
+    sig = O.sigma_table(o.sigma, o.sigma_nmax, nmax, mode)
+    sel = np.arange(x.shape[0]) if rows is None else np.asarray(sorted(rows))
+    xs = np.ascontiguousarray(x[sel])
+    o_snr, o_w, o_m = O.sweep(xs, o.mean, sig)
+    g_snr = snr[torch.from_numpy(sel).cuda()].cpu().numpy(); g_w = width[torch.from_numpy(sel).cuda()].cpu().numpy()
+    r = CMP.compare_planes(xs, o.mean, sig, g_snr, g_w, o_snr, o_w, o_m)
+    assert r, str(r)
+    # candidates restricted to the compared rows
+    pos = {int(s): i for i, s in enumerate(sel)}
+    m = np.isin(rec["dm"], sel)
+    dm_local = np.array([pos[int(v)] for v in rec["dm"][m]], dtype=np.int64)
+    rc = CMP.compare_candidates(dm_local, rec["t"][m], rec["snr"][m], rec["width"][m], int(m.sum()), 1 << 22,
+                                o_snr, o_w, o_m, cfg.threshold)
+    assert rc, str(rc)
+    if fused:
+        rec2, total2 = gpu_fused(d, st, nmax, mode, cfg.threshold, capacity=1 << 22)
+        assert total2 == total
+        assert np.sort(rec, order=["dm", "t"]).tobytes() == np.sort(rec2, order=["dm", "t"]).tobytes()
+    return rec, total, r, rc
+
+
+def test_config1_whole_path(P):
+    cfg = gen.get_config(1)
+    x = gen.make_array(cfg)
+    rec, total, r, rc = _whole_path(P, cfg, x, cfg.nmax[0])
+    for p in gen.pulse_table(cfg):                     # every injected pulse is recovered at (about) its width
+        sel = (rec["dm"] == p.row) & (np.abs(rec["t"].astype(np.int64) - p.start) <= cfg.nmax[0])
+        assert sel.any(), p
+        k = np.argmax(np.where(sel, rec["snr"], -np.inf))
+        assert abs(rec["snr"][k] - p.snr) < 3.0 and 0.5 * p.width <= rec["width"][k] <= 2 * p.width + 1
+
+
+def test_config2_whole_path_full_size(P):
+    cfg = gen.get_config(2)
+    x = gen.make_array(cfg)
+    rows = sorted(set(gen.pulse_rows(cfg)) | set(range(0, cfg.n_dm, 64)))
+    _whole_path(P, cfg, x, cfg.nmax[0], rows=rows)
+
+
+def test_search_host_matches_device_calls(P):
+    cfg = gen.get_config(1)
+    x = gen.make_array(cfg)
+    nmax, cap = cfg.nmax[0], 4096
+    h_x = torch.from_numpy(x).pin_memory()
+    h_out = torch.zeros((cap, 4), dtype=torch.int32).pin_memory()
+    h_count = torch.zeros(1, dtype=torch.int64).pin_memory()
+    h_stats = torch.zeros(P.STATS_DTYPE.itemsize, dtype=torch.uint8).pin_memory()
+    arena = torch.empty(P.search_host_arena_bytes(cfg.n_dm, cfg.n_t, nmax, cap), dtype=torch.uint8, device="cuda")
+    total = P.spd_search_host(h_x, nmax, "sqrt", cfg.threshold, h_out, h_count, h_stats, arena)
+    rec = h_out[:total].numpy().view(P.CAND_DTYPE).reshape(-1)
+    d = torch.from_numpy(x).cuda()
+    st = P.spd_stats(d)
+    snr, width = P.spd_boxcar_snr(d, st, nmax, "sqrt")
+    out, cnt = P.spd_candidates(snr, width, cfg.threshold, capacity=cap)
+    rec2, total2 = P.read_candidates(out, cnt)
+    assert total == total2 and total > 0
+    assert np.sort(rec, order=["dm", "t"]).tobytes() == np.sort(rec2, order=["dm", "t"]).tobytes()
+    assert h_stats.numpy().tobytes() == st.cpu().numpy().tobytes()
+
+
+def test_argument_errors_on_device(P):
+    x = torch.zeros((2, 100), device="cuda")
+    st = P.write_stats(0.0, 1.0)
+    with pytest.raises(P.SpdError):
+        P.spd_boxcar_snr(x, st, 101)                  # nmax > n_t
+    with pytest.raises(P.SpdError):
+        P.spd_boxcar_snr(x, st, 0)
+    with pytest.raises(P.SpdError):
+        P.spd_stats(x, 5000)
+    with pytest.raises(P.SpdError):
+        P.spd_boxcar_snr(x, st, 8, ws=torch.empty(16, dtype=torch.uint8, device="cuda"))   # SPD_ERR_WORKSPACE
