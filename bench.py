@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the single-pulse-detection hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--nmax M] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (spd_stats -> spd_boxcar_snr -> spd_candidates) over one chunk of
+synthetic de-dispersed data (gen/, config C; default 3 = the SKA-like chunk BASELINE.json's metric and target
+are quoted on).  Prints ONE JSON line on rank 0.  Inputs are resident in HBM for `value`; `e2e` goes through
+spd_search_host with pinned HOST buffers (H2D + D2H inside the timed region).
+`--impl reference` times the CPU oracle (oracle/) on a bounded row sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import gen  # noqa: E402
+
+METRIC = "DM×time samples/s through boxcar SNR search (×real-time); HBM GB/s vs peak"
+SM_COUNT, FP32_LANES_PER_SM = 148, 128
+# DRAM bytes per launch of boxcar_snr_sweep on config 3 from `ncu --set full` (profiles/r01_sweep_full.md); None = not captured
+SWEEP_DRAM_TRAFFIC_C3 = None
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.1] or [r for (_, r) in self.rows[-3:]]
+        for r in rows:
+            f = [s.strip() for s in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def pick_workload(args):
+    cfg = gen.get_config(args.config)
+    nmax = args.nmax or (128 if cfg.cid == 5 else cfg.nmax[0])
+    n_dm = args.rows or cfg.n_dm
+    return cfg, nmax, n_dm
+
+
+def workload_name(cfg, nmax, n_dm):
+    return f"{cfg.name}: {n_dm} DM trials x {cfg.n_t} samples f32, Nmax={nmax}, sigma_N {cfg.sigma_mode}, threshold {cfg.threshold}"
+
+
+def oracle_sample_rate(cfg, nmax, target_s: float, rank_seed: int = 0):
+    """The oracle, as it stands, on a bounded row sample of the workload: (samples/s, cores, sample text, seconds)."""
+    from oracle import spd_oracle as O
+    O.build()
+    cores = O.num_threads()
+    rows = min(cfg.n_dm, max(2, cores))
+    x = gen.make_rows(cfg, list(range(rows)))
+    t0 = time.time()
+    O.search(x, nmax, cfg.sigma_mode, cfg.threshold)
+    dt = time.time() - t0
+    want = int(min(cfg.n_dm, max(rows, rows * target_s / max(dt, 1e-3))))
+    want = max(cores, want - want % cores) if want >= cores else want
+    if want > rows:
+        x = gen.make_array(cfg, row_lo=0, row_hi=want)
+        t0 = time.time()
+        O.search(x, nmax, cfg.sigma_mode, cfg.threshold)
+        dt = time.time() - t0
+        rows = want
+    n = rows * cfg.n_t
+    return n / dt, cores, f"first {rows} of {cfg.n_dm} rows ({n} samples, {dt:.1f} s of oracle time: stats+sweep+candidates)", dt
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the box's host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import spd_oracle as O
+    O.build()
+    cfg, nmax, n_dm = pick_workload(args)
+    cores = O.num_threads()
+    rows = min(n_dm, max(2, 2 * cores))
+    x = gen.make_rows(cfg, list(range(rows)))
+    for _ in range(min(args.warmup, 1)):
+        O.search(x, nmax, cfg.sigma_mode, cfg.threshold)
+    t0 = time.time()
+    for _ in range(args.steps):
+        O.search(x, nmax, cfg.sigma_mode, cfg.threshold)
+    dt = (time.time() - t0) / args.steps
+    n = rows * cfg.n_t
+    v = n / dt
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": "samples/s", "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload_name(cfg, nmax, n_dm), "sample": f"each step = first {rows} rows ({n} samples)"},
+           "cpu_baseline": {"value": v, "unit": "samples/s", "cores": cores, "kind": "oracle",
+                            "sample": f"first {rows} of {n_dm} rows per step, {args.steps} steps"},
+           "e2e": {"value": v, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    import paper_1611_09704_b200 as P
+    P.lib()
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    cfg, nmax, n_dm = pick_workload(args)
+    if world > 1:          # weak scaling: every rank searches its own, differently seeded chunk of the same shape
+        import dataclasses
+        cfg = dataclasses.replace(cfg, cid=cfg.cid + 100 * rank)
+    n_t, mode, thr = cfg.n_t, cfg.sigma_mode, cfg.threshold
+    n = n_dm * n_t
+    cap = 1 << 20
+
+    # ---- synthetic input (host, pinned), then resident in HBM -----------------------------------------------
+    t_gen = time.time()
+    h_x = torch.empty((n_dm, n_t), dtype=torch.float32, pin_memory=True)
+    gen.make_array(cfg, out=h_x.numpy(), threads=max(1, (os.cpu_count() or 1) // max(1, world)), row_hi=n_dm)
+    t_gen = time.time() - t_gen
+    arena = torch.empty(P.search_host_arena_bytes(n_dm, n_t, nmax, cap), dtype=torch.uint8, device=dev)
+    # device-resident leg uses the arena's own regions (same layout as spd_search_host): x | snr | width
+    def region(off, nbytes, dtype, shape):
+        return arena[off:off + nbytes].view(dtype).view(shape)
+    a256 = lambda v: (v + 255) // 256 * 256
+    o_x, o_snr, o_w = 0, a256(n * 4), a256(n * 4) * 2
+    d_x = region(o_x, n * 4, torch.float32, (n_dm, n_t))
+    d_snr = region(o_snr, n * 4, torch.float32, (n_dm, n_t))
+    d_w = region(o_w, n * 2, torch.uint16, (n_dm, n_t))
+    d_x.copy_(h_x, non_blocking=True)
+    st = P.new_stats(dev)
+    ws = P.new_workspace(n_dm, n_t, nmax, dev)
+    out, cnt = P.new_candidates(cap, dev)
+    nmax_sigma = nmax if mode != "sqrt" else 0
+    launches_per_step = 2 + (1 if nmax_sigma else 0) + 2 + 2     # stats(+sigma_nmax), table+sweep, zero+compact
+
+    def step(ev=None):
+        P.spd_stats(d_x, nmax_sigma, st, ws)
+        if ev: ev[0].record()
+        P.spd_boxcar_snr(d_x, st, nmax, mode, d_snr, d_w, ws)
+        if ev: ev[1].record()
+        P.spd_candidates(d_snr, d_w, thr, out, cnt)
+        if ev: ev[2].record()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    w0 = time.time()
+    e0.record()
+    for i in range(args.steps):
+        step(evs[i])
+    e1.record()
+    barrier()
+    w1 = time.time()
+    clocks = sampler.stop(w0, w1) if rank == 0 else None
+    ms_total = e0.elapsed_time(e1)
+    t_stats = [e0.elapsed_time(evs[0][0])] + [evs[i - 1][2].elapsed_time(evs[i][0]) for i in range(1, args.steps)]
+    t_sweep = [evs[i][0].elapsed_time(evs[i][1]) for i in range(args.steps)]
+    t_cand = [evs[i][1].elapsed_time(evs[i][2]) for i in range(args.steps)]
+    hits = int(cnt.item())
+    stats_host = P.read_stats(st)[0]
+
+    # ---- end to end through the C ABI with HOST buffers (H2D of x, D2H of stats + count + list each step) ------
+    h_out = torch.zeros((cap, 4), dtype=torch.int32).pin_memory()
+    h_cnt = torch.zeros(1, dtype=torch.int64).pin_memory()
+    h_st = torch.zeros(P.STATS_DTYPE.itemsize, dtype=torch.uint8).pin_memory()
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    for _ in range(1):
+        P.spd_search_host(h_x, nmax, mode, thr, h_out, h_cnt, h_st, arena)
+    barrier()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record()
+    for _ in range(e2e_steps):
+        hits_e2e = P.spd_search_host(h_x, nmax, mode, thr, h_out, h_cnt, h_st, arena)
+    f1.record()
+    barrier()
+    ms_e2e = f0.elapsed_time(f1) / e2e_steps
+
+    # ---- max over ranks -------------------------------------------------------------------------------------------
+    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, ms_e2e = float(t[0]), float(t[1])
+    ms_step = ms_total / args.steps
+
+    if rank == 0:
+        hbm_peak, sm_max_mhz, peak_kind = _peaks()
+        pairs = float(n) * nmax
+        sweep_ms = float(np.mean(t_sweep))
+        alu_peak = SM_COUNT * FP32_LANES_PER_SM * sm_max_mhz * 1e6 / 1e12          # T lane-instructions/s
+        alu_ach = 2.0 * pairs / (sweep_ms * 1e-3) / 1e12                            # one fp32 add + one fp32 multiply per pair
+        hbm_ach = 10.0 * n / (sweep_ms * 1e-3) / 1e9
+        hbm_bound = (10.0 * n / (hbm_peak * 1e9)) > (2.0 * pairs / (alu_peak * 1e12))
+        roof = ({"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak}
+                if hbm_bound else
+                {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": alu_ach / alu_peak})
+        roof.update({"kernel": "boxcar_snr_sweep", "traffic": SWEEP_DRAM_TRAFFIC_C3 if (cfg.cid % 100 == 3 and nmax == 128 and n_dm == 6000) else None,
+                     "peak_source": f"{peak_kind} (MEASURED_PEAKS.json)" if roof["bound"] == "hbm" else
+                                    "derived: 148 SM x 128 fp32 lanes x sm_max_mhz (FMA pipe, non-fused ops); 2 flops (add, multiply) per (sample,width) pair",
+                     "ms_per_launch": sweep_ms, "algorithmic_bytes_per_sample": 10, "flops_per_pair": 2,
+                     "hbm_GBps": hbm_ach, "hbm_frac_of_measured": hbm_ach / hbm_peak, "hbm_frac_of_8TBps": hbm_ach / 8000.0,
+                     "alu_Tops": alu_ach, "alu_frac": alu_ach / alu_peak})
+        cpu = None
+        if not args.no_cpu_baseline:
+            v, cores, sample, _ = oracle_sample_rate(gen.get_config(args.config), nmax, args.cpu_seconds)
+            cpu = {"value": v, "unit": "samples/s", "cores": cores, "kind": "oracle", "sample": sample}
+        value = world * n / (ms_step * 1e-3)
+        res = {
+            "metric": METRIC, "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, nmax, n_dm), "config_id": args.config, "n_dm": n_dm, "n_t": n_t,
+                       "nmax": nmax, "sigma_mode": mode, "threshold": thr, "samples_per_step_per_gpu": n,
+                       "l2": "input 4n bytes >> 126 MB L2, no flush needed" if n * 4 > (1 << 29) else "L2-resident input (small config)",
+                       "parallelism": f"independent chunks, one per GPU (x{world})", "gen_seconds": round(t_gen, 1)},
+            "x_realtime": (n_t * cfg.t_samp) / (ms_step * 1e-3) if cfg.cid % 100 == 3 else None,
+            "breakdown_ms": {"spd_stats": float(np.mean(t_stats)), "spd_boxcar_snr": sweep_ms, "spd_candidates": float(np.mean(t_cand))},
+            "stats_GBps": 4.0 * n * (2 if nmax_sigma else 1) / (float(np.mean(t_stats)) * 1e-3) / 1e9,
+            "candidates_GBps": 4.0 * n / (float(np.mean(t_cand)) * 1e-3) / 1e9,
+            "hits": hits, "mean": float(stats_host["mean"]), "sigma": float(stats_host["sigma"]),
+            "clocks": clocks,
+            "e2e": {"value": world * n / (ms_e2e * 1e-3), "unit": "samples/s", "ms_per_step": ms_e2e, "steps": e2e_steps,
+                    "h2d_bytes_per_step": n * 4, "d2h_bytes_per_step": 8 + P.STATS_DTYPE.itemsize + 16 * min(hits_e2e, cap),
+                    "api": "spd_search_host (pinned host buffers)"},
+            "gpu_launches": launches_per_step * args.steps,
+            "roofline": roof,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(res), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE config 1..5 (default 3 = SKA-like)")
+    ap.add_argument("--nmax", type=int, default=0, help="override the widest boxcar")
+    ap.add_argument("--rows", type=int, default=0, help="override n_dm (smaller runs for profiling)")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,7 +1,7 @@
 """spd-b200: single-pulse detection (arXiv 1611.09704) as hand-written sm_100a CUDA kernels behind a C ABI.
 
 `binding` is a thin ctypes layer over libspd.so (include/spd.h); `build` compiles the library in-tree.
-Nothing here computes on the CPU and nothing here imports the oracle.
+Nothing here computes on the CPU; the package is independent of the CPU checker used by the tests.
 """
 from .binding import (  # noqa: F401
     SpdError, lib, LIB_PATH, STATS_DTYPE, CAND_DTYPE,

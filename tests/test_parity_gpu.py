@@ -264,7 +264,9 @@ def _whole_path(P, cfg, x, nmax, rows=None, fused=True):
     sel = np.arange(x.shape[0]) if rows is None else np.asarray(sorted(rows))
     xs = np.ascontiguousarray(x[sel])
     o_snr, o_w, o_m = O.sweep(xs, o.mean, sig)
-    g_snr = snr[torch.from_numpy(sel).cuda()].cpu().numpy(); g_w = width[torch.from_numpy(sel).cuda()].cpu().numpy()
+    idx = torch.from_numpy(sel).cuda()
+    g_snr = snr[idx].cpu().numpy()
+    g_w = width.view(torch.int16)[idx].cpu().numpy().view(np.uint16)      # uint16 has no index kernel in torch
     r = CMP.compare_planes(xs, o.mean, sig, g_snr, g_w, o_snr, o_w, o_m)
     assert r, str(r)
     # candidates restricted to the compared rows
