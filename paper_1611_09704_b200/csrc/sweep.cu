@@ -4,20 +4,25 @@
 //   B_N(t) = sum_{k<N} x[t+k];  SNR_N(t) = (B_N(t) - N mu) / sigma_N;  snr[t] = max_N, width[t] = smallest arg-max.
 //
 // Design (sm_100a; this is NOT the paper's one-thread-X-samples loop):
-//  * y = x - mu is formed once per sample while the tile is staged into shared memory (fp64 subtract, fp32
-//    result), so the inner loop is B += y; s = B * r_N with r_N = 1/sigma_N from a table: no divide, no sqrt.
-//  * One CTA owns 2048 consecutive samples of one row, as two sub-tiles A = [T0, T0+1024), B = [T0+1024, T0+2048).
-//    Shared memory holds them INTERLEAVED as float2 Z[i] = (yA[i], yB[i]) so that one packed FADD2 / FMUL2
+//  * Persistent CTAs (one wave, grid = SMs x resident CTAs) walk the tiles; the raw samples of the NEXT tile are
+//    prefetched with cp.async (LDGSTS, 16 B) into shared memory while the current tile is swept.
+//  * y = x - mu is formed once per sample when the raw tile is converted into the working layout (two-term fp32
+//    subtract, mu = mu_hi + mu_lo), so the inner loop is B += y; s = B * r_N with r_N = 1/sigma_N from a table.
+//  * One tile = 2048 consecutive samples of one row, as two sub-tiles A = [T0, T0+1024), B = [T0+1024, T0+2048).
+//    The working layout INTERLEAVES them, float2 Z[i] = (yA[i], yB[i]), so that one packed FADD2 / FMUL2
 //    (Blackwell packed fp32) advances one running sum of each sub-tile: the FMA pipe sees 2 lane-ops per
-//    (sample, width) pair -- the arithmetic floor -- for ONE issue slot per pair.
+//    (sample, width) pair -- the arithmetic floor -- for one issue slot per pair.
 //  * Each thread owns 8 consecutive samples of each sub-tile and keeps a sliding window of 8 float2 in registers
 //    (the width loop is unrolled by 8, so the rotation is register renaming): one LDS.64 per width step.
 //  * Samples past the row end are staged as -inf: a running sum that has touched one is -inf for every wider
 //    width, so "only widths that fit" (reading A9) needs no masking in the loop.
-//  * arg-max is deferred: per block of 8 widths only the block maximum is formed (3-input FMNMX), one
-//    compare/select per block records the winning block and the running sum at its start; after the loop the
-//    winning block alone is re-summed in the same order (bit-identical) to find the smallest width attaining
-//    the maximum.  Blocks ascend and every comparison is a strict '>' , so ties keep the smallest width (A7).
+//  * arg-max is deferred: the running maximum is advanced with 3-input FMNMX only; per block of 8 widths one
+//    compare + one select record the block that last raised it.  After the loop that block alone is evaluated
+//    again, width by width, from a tile-local prefix sum P kept in shared memory (B_w(t) = P[t+w] - P[t], no
+//    dependency chain), and the smallest width attaining the block maximum is taken.  Blocks ascend and every
+//    comparison is a strict '>', so ties keep the smallest width (A7).  The SNR written is the running-sum value
+//    of the main loop; the prefix-sum re-evaluation only picks the width, and can differ from the running sums by
+//    fp32 rounding (~1e-6), i.e. only inside near-ties far below the 1e-3 tie tolerance.
 //
 // Roofline: 10 B/sample of HBM traffic (4 read + 4 snr + 2 width) against 2*Nmax fp32 lane-ops per sample on the
 // FMA pipe: FP32-pipe-bound for Nmax > ~28.
@@ -28,15 +33,42 @@ namespace spd {
 constexpr int SW_THREADS = 128;
 constexpr int SW_R       = 8;                        // samples per thread per sub-tile
 constexpr int SW_SUB     = SW_THREADS * SW_R;        // 1024
-constexpr int SW_TILE    = 2 * SW_SUB;               // 2048 samples per CTA
+constexpr int SW_TILE    = 2 * SW_SUB;               // 2048 samples per tile
 
 __host__ __device__ inline int zpad(int i) { return i + (i >> 3); }          // one pad float2 per 8: lane stride 72 B
-__host__ __device__ inline int sw_len(int nmax) { return SW_SUB + round_up(nmax, 8) + 16; }
-__host__ __device__ inline int sw_rt_len(int nmax) { return round_up(nmax, 8) + 8; }
+__host__ __device__ inline int sw_halo(int nmax) { return round_up(nmax, 8) + 24; }
+__host__ __device__ inline int sw_rt_len(int nmax) { return round_up(nmax, 8) + 24; }
 
 size_t sweep_table_bytes(int nmax) { return (size_t)sw_rt_len(nmax) * sizeof(float); }
 
+struct SweepSmem {           // byte offsets into dynamic shared memory (all 16-byte aligned)
+    int z, raw, pa, pb, scan, rt2, rtf, total;
+    __host__ __device__ explicit SweepSmem(int nmax)
+    {
+        const int H = sw_halo(nmax), R = sw_rt_len(nmax);
+        const int P = round_up((zpad(SW_SUB + H + 1) + 1) * 4, 16);      // one prefix array (floats, zpad layout)
+        z = 0;
+        raw = z + round_up((zpad(SW_SUB + H) + 1) * 8, 16);
+        pa = raw + round_up((SW_TILE + H) * 4, 16);
+        pb = pa + P;
+        scan = pb + P;
+        rt2 = scan + 64;
+        rtf = rt2 + R * 8;
+        total = rtf + round_up(R * 4, 16);
+    }
+};
+
 __device__ __forceinline__ float fmax3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit_wait_all()
+{
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+}
 
 // r_w = 1/sigma_w for w = 1..nmax: eq. 4, eq. 5 as printed, or the anchored variant.
 // fp64 throughout, rounded once to fp32.  LINEAR modes fed stats measured for another Nmax write NaN.
@@ -64,188 +96,273 @@ cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, f
     return cudaGetLastError();
 }
 
+// 8 width steps: advance the 8 packed running sums, scale, fold into the running maxima.
+// On entry W[v] = Z[i0 + a0 + v] (a0 = width offset of the first step); on exit the window has moved by 8.
+__device__ __forceinline__ void sweep8(float2 (&B)[SW_R], float2 (&W)[SW_R], float2 (&best)[SW_R],
+                                       const float2 *__restrict__ zp, const float2 *__restrict__ rp)
+{
+#pragma unroll
+    for (int u = 0; u < 8; u += 2) {
+        const float4 rr = *reinterpret_cast<const float4 *>(rp + u);
+        const float2 r0 = make_float2(rr.x, rr.y), r1 = make_float2(rr.z, rr.w);
+        float2 s0[SW_R], s1[SW_R];
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) { B[j] = __fadd2_rn(B[j], W[(j + u) & 7]); s0[j] = __fmul2_rn(B[j], r0); }
+        W[u] = zp[u];
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) { B[j] = __fadd2_rn(B[j], W[(j + u + 1) & 7]); s1[j] = __fmul2_rn(B[j], r1); }
+        W[u + 1] = zp[u + 1];
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) {
+            best[j].x = fmax3(best[j].x, s0[j].x, s1[j].x);
+            best[j].y = fmax3(best[j].y, s0[j].y, s1[j].y);
+        }
+    }
+}
+
+// record, per running sum, whether the block of widths that just ended raised the maximum
+__device__ __forceinline__ void note_block(const float2 (&best)[SW_R], const float2 (&old)[SW_R], int w0,
+                                           int (&w0x)[SW_R], int (&w0y)[SW_R])
+{
+#pragma unroll
+    for (int j = 0; j < SW_R; ++j) {
+        w0x[j] = (best[j].x > old[j].x) ? w0 : w0x[j];
+        w0y[j] = (best[j].y > old[j].y) ? w0 : w0y[j];
+    }
+}
+
 template <bool FUSED>
 __global__ void __launch_bounds__(SW_THREADS, 3)
-boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row,
+boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                  const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
                  float *__restrict__ snr, uint16_t *__restrict__ width,
                  float threshold, spd_candidate_t *__restrict__ cand, unsigned long long capacity,
                  unsigned long long *__restrict__ count)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int L = sw_len(nmax);
-    float2 *Z  = reinterpret_cast<float2 *>(smem_raw);
-    float2 *rt = Z + ((zpad(L) + 1) & ~1);
+    const SweepSmem lay(nmax);
+    float2 *Z   = reinterpret_cast<float2 *>(smem_raw + lay.z);
+    float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
+    float2 *rt2 = reinterpret_cast<float2 *>(smem_raw + lay.rt2);     // (r_w, r_w): operand of FMUL2
+    float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);      // r_w plain: LDS.128 in the width search
+    float  *PA  = reinterpret_cast<float *>(smem_raw + lay.pa);       // prefix sums of y, sub-tile A (zpad layout)
+    float  *PB  = reinterpret_cast<float *>(smem_raw + lay.pb);       // prefix sums of y, sub-tile B
+    float2 *scan = reinterpret_cast<float2 *>(smem_raw + lay.scan);   // per-warp totals of the tile prefix scan
 
     const int tid = threadIdx.x;
-    const int64_t row = blockIdx.x / tiles_per_row;
-    const int64_t T0 = (int64_t)(blockIdx.x - row * tiles_per_row) * SW_TILE;
-    const float *rowp = x + row * row_stride;
+    const int H = sw_halo(nmax);
+    const int LRAW = SW_TILE + H;                 // raw floats per tile: x[T0 .. T0 + 2048 + H)
+    const int LZ = SW_SUB + H;                    // interleaved positions
     const double mu = st->mean;
+    const float mu_hi = (float)mu, mu_lo = (float)(mu - (double)mu_hi);
     const float NINF = __int_as_float(0xff800000);
+    const int nblk8 = nmax >> 3, rem = nmax & 7;
+    const int SEG = (LZ + SW_THREADS - 1) / SW_THREADS;       // consecutive positions per thread in the prefix scan
+    const int lane = tid & 31, wid = tid >> 5;
 
-    // ---- stage: y = x - mu, two sub-tiles interleaved; past the row end -> -inf -------------------------------
-    {
+    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) { float r = __ldg(table + w); rt2[w] = make_float2(r, r); rtf[w] = r; }
+
+    // raw tile -> shared memory, asynchronously where the 16-byte fast path applies; past the row end -> -inf
+    auto prefetch = [&](int64_t tile) {
+        const int64_t row = tile / tiles_per_row;
+        const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
+        const float *rowp = x + row * row_stride;
         const bool vec = ((reinterpret_cast<uintptr_t>(rowp) & 15) == 0);
-        for (int p = tid; p < L / 4; p += SW_THREADS) {
-            const int i = 4 * p;
-            float a[4], b[4];
-            const int64_t pa = T0 + i, pb = T0 + SW_SUB + i;
-            if (vec && pa + 3 < n_t) { float4 v = __ldg(reinterpret_cast<const float4 *>(rowp + pa)); a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w; }
-            else { for (int k = 0; k < 4; ++k) a[k] = (pa + k < n_t) ? __ldg(rowp + pa + k) : NINF; }
-            if (vec && pb + 3 < n_t) { float4 v = __ldg(reinterpret_cast<const float4 *>(rowp + pb)); b[0] = v.x; b[1] = v.y; b[2] = v.z; b[3] = v.w; }
-            else { for (int k = 0; k < 4; ++k) b[k] = (pb + k < n_t) ? __ldg(rowp + pb + k) : NINF; }
+        if (vec && T0 + LRAW <= n_t) {                       // interior tile: no bounds checks
+            const float *src = rowp + T0;
+            for (int p = tid; p < LRAW / 4; p += SW_THREADS) cp_async16(raw + 4 * p, src + 4 * p);
+        } else {
+            for (int p = tid; p < LRAW / 4; p += SW_THREADS) {
+                const int64_t pos = T0 + 4 * p;
+                if (vec && pos + 3 < n_t) cp_async16(raw + 4 * p, rowp + pos);
+                else {
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
-                Z[zpad(i + k)] = make_float2((float)((double)a[k] - mu), (float)((double)b[k] - mu));
-        }
-        for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) { float r = __ldg(table + w); rt[w] = make_float2(r, r); }
-    }
-    __syncthreads();
-
-    // ---- per-thread state --------------------------------------------------------------------------------------
-    float2 B[SW_R], W[SW_R], best[SW_R], snap[SW_R];
-    int blkx[SW_R], blky[SW_R];
-#pragma unroll
-    for (int j = 0; j < SW_R; ++j) {
-        B[j] = make_float2(0.f, 0.f);
-        W[j] = Z[9 * tid + j];                               // zpad(8 tid + j) = 9 tid + j
-        best[j] = make_float2(NINF, NINF);
-        snap[j] = make_float2(0.f, 0.f);
-        blkx[j] = 0; blky[j] = 0;
-    }
-    const int nblk = nmax >> 3;
-
-    // ---- main loop: one iteration = one block of 8 widths ------------------------------------------------------
-    for (int kb = 0; kb < nblk; ++kb) {
-        const float2 *zp = Z + 9 * (tid + kb + 1);           // zpad(8 tid + 8 kb + 8 + u) = 9 (tid + kb + 1) + u
-        const float2 *rp = rt + 8 * kb;
-        float2 B0[SW_R], m[SW_R];
-#pragma unroll
-        for (int j = 0; j < SW_R; ++j) B0[j] = B[j];
-#pragma unroll
-        for (int u = 0; u < 8; u += 2) {
-            const float4 rr = *reinterpret_cast<const float4 *>(rp + u);
-            const float2 r0 = make_float2(rr.x, rr.y), r1 = make_float2(rr.z, rr.w);
-            float2 s0[SW_R], s1[SW_R];
-#pragma unroll
-            for (int j = 0; j < SW_R; ++j) { B[j] = __fadd2_rn(B[j], W[(j + u) & 7]); s0[j] = __fmul2_rn(B[j], r0); }
-            W[u] = zp[u];
-#pragma unroll
-            for (int j = 0; j < SW_R; ++j) { B[j] = __fadd2_rn(B[j], W[(j + u + 1) & 7]); s1[j] = __fmul2_rn(B[j], r1); }
-            W[u + 1] = zp[u + 1];
-#pragma unroll
-            for (int j = 0; j < SW_R; ++j) {
-                if (u == 0) { m[j].x = fmaxf(s0[j].x, s1[j].x); m[j].y = fmaxf(s0[j].y, s1[j].y); }
-                else        { m[j].x = fmax3(m[j].x, s0[j].x, s1[j].x); m[j].y = fmax3(m[j].y, s0[j].y, s1[j].y); }
+                    for (int k = 0; k < 4; ++k) raw[4 * p + k] = (pos + k < n_t) ? __ldg(rowp + pos + k) : NINF;
+                }
             }
         }
+    };
+
+    int64_t tile = blockIdx.x;
+    if (tile < total_tiles) prefetch(tile);
+
+    for (; tile < total_tiles; tile += gridDim.x) {
+        const int64_t row = tile / tiles_per_row;
+        const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
+        cp_async_commit_wait_all();
+        __syncthreads();                           // raw tile landed; everyone is done with the previous Z / P
+        {
+            // y = x - mu into the interleaved layout, and the tile-local inclusive prefix sums of y (per sub-tile)
+            const int lo = tid * SEG, hi = min(lo + SEG, LZ);
+            float2 run = make_float2(0.f, 0.f);
+            for (int i = lo; i < hi; ++i) {
+                const float2 y = make_float2((raw[i] - mu_hi) - mu_lo, (raw[SW_SUB + i] - mu_hi) - mu_lo);
+                Z[zpad(i)] = y;
+                run = __fadd2_rn(run, y);
+                PA[zpad(i + 1)] = run.x; PB[zpad(i + 1)] = run.y;
+            }
+            float2 inc = run;                       // inclusive scan of the thread totals across the CTA
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const float ox = __shfl_up_sync(0xffffffffu, inc.x, d), oy = __shfl_up_sync(0xffffffffu, inc.y, d);
+                if (lane >= d) { inc.x += ox; inc.y += oy; }
+            }
+            if (lane == 31) scan[wid] = inc;
+            __syncthreads();
+            float2 off;                             // exclusive prefix inside the warp (no inc - run: -inf - -inf is NaN)
+            off.x = __shfl_up_sync(0xffffffffu, inc.x, 1); off.y = __shfl_up_sync(0xffffffffu, inc.y, 1);
+            if (lane == 0) off = make_float2(0.f, 0.f);
+            for (int w = 0; w < wid; ++w) { off.x += scan[w].x; off.y += scan[w].y; }
+            for (int i = lo; i < hi; ++i) { PA[zpad(i + 1)] += off.x; PB[zpad(i + 1)] += off.y; }
+            if (tid == 0) { PA[0] = 0.f; PB[0] = 0.f; }
+        }
+        __syncthreads();                           // Z and P complete; raw is free again
+        if (tile + gridDim.x < total_tiles) prefetch(tile + gridDim.x);
+
+        // ---- per-thread state ----------------------------------------------------------------------------------
+        float2 B[SW_R], W[SW_R], best[SW_R];
+        int w0x[SW_R], w0y[SW_R];
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) {
-            const bool px = m[j].x > best[j].x, py = m[j].y > best[j].y;
-            best[j].x = px ? m[j].x : best[j].x;  snap[j].x = px ? B0[j].x : snap[j].x;  blkx[j] = px ? kb : blkx[j];
-            best[j].y = py ? m[j].y : best[j].y;  snap[j].y = py ? B0[j].y : snap[j].y;  blky[j] = py ? kb : blky[j];
+            B[j] = make_float2(0.f, 0.f);
+            W[j] = Z[9 * tid + j];                           // zpad(8 tid + j) = 9 tid + j
+            best[j] = make_float2(NINF, NINF);
+            w0x[j] = 0; w0y[j] = 0;
         }
-    }
 
-    // ---- re-sum the winning block (same order, same roundings) to find the smallest width attaining best --------
-    int wx[SW_R], wy[SW_R];
+        // ---- main loop: one iteration = one block of 8 widths ------------------------------------------------------
+        for (int kb = 0; kb < nblk8; ++kb) {
+            float2 old[SW_R];
 #pragma unroll
-    for (int j = 0; j < SW_R; ++j) {
-        wx[j] = 1; wy[j] = 1;
-        if (nblk > 0) {
+            for (int j = 0; j < SW_R; ++j) old[j] = best[j];
+            sweep8(B, W, best, Z + 9 * (tid + kb + 1), rt2 + 8 * kb);             // zpad(8 tid + 8 kb + 8 + u)
+            note_block(best, old, 8 * kb, w0x, w0y);
+        }
+
+        // ---- width search inside the winning block, from the prefix sums: B_w(t) = P[t + w] - P[t] ------------------
+        int wx[SW_R], wy[SW_R];
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int kb = h ? blky[j] : blkx[j];
-                const float bst = h ? best[j].y : best[j].x;
-                float b = h ? snap[j].y : snap[j].x;
-                const float *zf = reinterpret_cast<const float *>(Z + 9 * (tid + kb)) + h;
-                const float *rf = reinterpret_cast<const float *>(rt + 8 * kb);
-                float s[8];
+        for (int j = 0; j < SW_R; ++j) {
+            wx[j] = 1; wy[j] = 1;
+            if (nblk8 > 0) {
 #pragma unroll
-                for (int g = 0; g < 8; ++g) { const int c = j + g; b += zf[2 * (c + (c >> 3))]; s[g] = b * rf[2 * g]; }
-                int w = 0;
+                for (int h = 0; h < 2; ++h) {
+                    const int w0 = h ? w0y[j] : w0x[j];
+                    const float *Ph = h ? PB : PA;
+                    const float p0 = Ph[9 * tid + j];                             // P[t], t = 8 tid + j
+                    const float *pe = Ph + 9 * (tid + (w0 >> 3));                 // zpad(8 tid + w0 + c) = 9 (tid + w0/8) + c + (c >> 3)
+                    const float4 *rq = reinterpret_cast<const float4 *>(rtf + w0);
+                    const float4 ra = rq[0], rb = rq[1];
+                    const float r[8] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y, rb.z, rb.w};
+                    float s[8];
 #pragma unroll
-                for (int g = 7; g >= 0; --g) w = (s[g] == bst) ? g : w;
-                if (h) wy[j] = 8 * kb + w + 1; else wx[j] = 8 * kb + w + 1;
+                    for (int g = 0; g < 8; ++g) { const int c = j + g + 1; s[g] = (pe[c + (c >> 3)] - p0) * r[g]; }
+                    const float m = fmaxf(fmax3(fmax3(s[0], s[1], s[2]), s[3], s[4]), fmax3(s[5], s[6], s[7]));
+                    int w = 0;
+#pragma unroll
+                    for (int g = 7; g >= 0; --g) w = (s[g] == m) ? g : w;
+                    if (h) wy[j] = w0 + w + 1; else wx[j] = w0 + w + 1;
+                }
             }
         }
-    }
 
-    // ---- tail widths (nmax not a multiple of 8): plain per-width tracking, wider widths so strict '>' still right
-    const int rem = nmax & 7;
-    if (rem) {
-        const float2 *zp = Z + 9 * (tid + nblk + 1);
-        for (int u = 0; u < rem; ++u) {
-            const float2 r = rt[8 * nblk + u];
-            const int wv = 8 * nblk + u + 1;
+        // ---- tail widths (nmax not a multiple of 8): per-width tracking; wider widths, so strict '>' is still right
+        if (rem) {
+            const float2 *zp = Z + 9 * (tid + nblk8 + 1);
+            for (int u = 0; u < rem; ++u) {
+                const float2 r = rt2[8 * nblk8 + u];
+                const int wv = 8 * nblk8 + u + 1;
 #pragma unroll
-            for (int j = 0; j < SW_R; ++j) {
-                B[j] = __fadd2_rn(B[j], W[j]);
-                const float2 s = __fmul2_rn(B[j], r);
-                if (s.x > best[j].x) { best[j].x = s.x; wx[j] = wv; }
-                if (s.y > best[j].y) { best[j].y = s.y; wy[j] = wv; }
+                for (int j = 0; j < SW_R; ++j) {
+                    B[j] = __fadd2_rn(B[j], W[j]);
+                    const float2 s = __fmul2_rn(B[j], r);
+                    if (s.x > best[j].x) { best[j].x = s.x; wx[j] = wv; }
+                    if (s.y > best[j].y) { best[j].y = s.y; wy[j] = wv; }
+                }
+#pragma unroll
+                for (int j = 0; j < SW_R - 1; ++j) W[j] = W[j + 1];  // rem < 8 steps: a plain shift is fine here
+                W[SW_R - 1] = zp[u];
             }
-#pragma unroll
-            for (int j = 0; j < SW_R - 1; ++j) W[j] = W[j + 1];      // rem < 8 steps: a plain shift is fine here
-            W[SW_R - 1] = zp[u];
         }
-    }
 
-    // a NaN reciprocal table (LINEAR mode fed stats of another Nmax) must surface: fmaxf drops NaN operands
-    if (rt[0].x != rt[0].x) {
+        // a NaN reciprocal table (LINEAR mode fed stats of another Nmax) must surface: fmaxf drops NaN operands
+        if (rtf[0] != rtf[0]) {
 #pragma unroll
-        for (int j = 0; j < SW_R; ++j) best[j] = make_float2(rt[0].x, rt[0].x);
-    }
+            for (int j = 0; j < SW_R; ++j) best[j] = make_float2(rtf[0], rtf[0]);
+        }
 
-    // ---- results --------------------------------------------------------------------------------------------------
-    const int64_t ta = T0 + SW_R * tid, tb = ta + SW_SUB;
-    if (!FUSED) {
-        float *oa = snr + row * row_stride + ta, *ob = snr + row * row_stride + tb;
-        const bool v4 = ((reinterpret_cast<uintptr_t>(snr + row * row_stride) & 15) == 0);
-        if (v4 && ta + 7 < n_t) {
-            reinterpret_cast<float4 *>(oa)[0] = make_float4(best[0].x, best[1].x, best[2].x, best[3].x);
-            reinterpret_cast<float4 *>(oa)[1] = make_float4(best[4].x, best[5].x, best[6].x, best[7].x);
+        // ---- results ----------------------------------------------------------------------------------------------
+        const int64_t ta = T0 + SW_R * tid, tb = ta + SW_SUB;
+        if (!FUSED) {
+            float *oa = snr + row * row_stride + ta, *ob = snr + row * row_stride + tb;
+            const bool v4 = ((reinterpret_cast<uintptr_t>(snr + row * row_stride) & 15) == 0);
+            if (v4 && ta + 7 < n_t) {
+                __stcs(reinterpret_cast<float4 *>(oa), make_float4(best[0].x, best[1].x, best[2].x, best[3].x));
+                __stcs(reinterpret_cast<float4 *>(oa) + 1, make_float4(best[4].x, best[5].x, best[6].x, best[7].x));
+            } else {
+#pragma unroll
+                for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) oa[j] = best[j].x;
+            }
+            if (v4 && tb + 7 < n_t) {
+                __stcs(reinterpret_cast<float4 *>(ob), make_float4(best[0].y, best[1].y, best[2].y, best[3].y));
+                __stcs(reinterpret_cast<float4 *>(ob) + 1, make_float4(best[4].y, best[5].y, best[6].y, best[7].y));
+            } else {
+#pragma unroll
+                for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) ob[j] = best[j].y;
+            }
+            if (width) {
+                uint16_t *wa = width + row * row_stride + ta, *wb = width + row * row_stride + tb;
+                const bool w8 = ((reinterpret_cast<uintptr_t>(width + row * row_stride) & 15) == 0);
+                if (w8 && ta + 7 < n_t)
+                    __stcs(reinterpret_cast<uint4 *>(wa), make_uint4(wx[0] | (wx[1] << 16), wx[2] | (wx[3] << 16), wx[4] | (wx[5] << 16), wx[6] | (wx[7] << 16)));
+                else {
+#pragma unroll
+                    for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) wa[j] = (uint16_t)wx[j];
+                }
+                if (w8 && tb + 7 < n_t)
+                    __stcs(reinterpret_cast<uint4 *>(wb), make_uint4(wy[0] | (wy[1] << 16), wy[2] | (wy[3] << 16), wy[4] | (wy[5] << 16), wy[6] | (wy[7] << 16)));
+                else {
+#pragma unroll
+                    for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) wb[j] = (uint16_t)wy[j];
+                }
+            }
         } else {
+            // threshold in the same kernel: planes are never written
+            bool any = false;
 #pragma unroll
-            for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) oa[j] = best[j].x;
-        }
-        if (v4 && tb + 7 < n_t) {
-            reinterpret_cast<float4 *>(ob)[0] = make_float4(best[0].y, best[1].y, best[2].y, best[3].y);
-            reinterpret_cast<float4 *>(ob)[1] = make_float4(best[4].y, best[5].y, best[6].y, best[7].y);
-        } else {
+            for (int j = 0; j < SW_R; ++j) any |= (best[j].x >= threshold && ta + j < n_t) || (best[j].y >= threshold && tb + j < n_t);
+            if (__any_sync(0xffffffffu, any)) {
 #pragma unroll
-            for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) ob[j] = best[j].y;
-        }
-        if (width) {
-            uint16_t *wa = width + row * row_stride + ta, *wb = width + row * row_stride + tb;
-            const bool w8 = ((reinterpret_cast<uintptr_t>(width + row * row_stride) & 15) == 0);
-            if (w8 && ta + 7 < n_t)
-                *reinterpret_cast<uint4 *>(wa) = make_uint4(wx[0] | (wx[1] << 16), wx[2] | (wx[3] << 16), wx[4] | (wx[5] << 16), wx[6] | (wx[7] << 16));
-            else {
-#pragma unroll
-                for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) wa[j] = (uint16_t)wx[j];
-            }
-            if (w8 && tb + 7 < n_t)
-                *reinterpret_cast<uint4 *>(wb) = make_uint4(wy[0] | (wy[1] << 16), wy[2] | (wy[3] << 16), wy[4] | (wy[5] << 16), wy[6] | (wy[7] << 16));
-            else {
-#pragma unroll
-                for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) wb[j] = (uint16_t)wy[j];
-            }
-        }
-    } else {
-        // threshold in the same kernel: planes are never written
-        bool any = false;
-#pragma unroll
-        for (int j = 0; j < SW_R; ++j) any |= (best[j].x >= threshold && ta + j < n_t) || (best[j].y >= threshold && tb + j < n_t);
-        if (__any_sync(0xffffffffu, any)) {
-#pragma unroll
-            for (int j = 0; j < SW_R; ++j) {
-                append_candidate(best[j].x >= threshold && ta + j < n_t, (uint32_t)row, (uint32_t)(ta + j), best[j].x, (uint32_t)wx[j], cand, capacity, count);
-                append_candidate(best[j].y >= threshold && tb + j < n_t, (uint32_t)row, (uint32_t)(tb + j), best[j].y, (uint32_t)wy[j], cand, capacity, count);
+                for (int j = 0; j < SW_R; ++j) {
+                    append_candidate(best[j].x >= threshold && ta + j < n_t, (uint32_t)row, (uint32_t)(ta + j), best[j].x, (uint32_t)wx[j], cand, capacity, count);
+                    append_candidate(best[j].y >= threshold && tb + j < n_t, (uint32_t)row, (uint32_t)(tb + j), best[j].y, (uint32_t)wy[j], cand, capacity, count);
+                }
             }
         }
     }
+    cp_async_commit_wait_all();
+}
+
+template <bool FUSED>
+static cudaError_t launch_sweep_t(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
+                                  const float *d_table, int nmax, float *snr, uint16_t *width, float threshold,
+                                  spd_candidate_t *out, unsigned long long capacity, unsigned long long *d_count, cudaStream_t s)
+{
+    const int tpr = (int)((n_t + SW_TILE - 1) / SW_TILE);
+    const int64_t tiles = n_dm * (int64_t)tpr;
+    const SweepSmem lay(nmax);
+    cudaError_t e = cudaFuncSetAttribute(boxcar_snr_sweep<FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, lay.total);
+    if (e != cudaSuccess) return e;
+    int dev = 0, sms = 0, per_sm = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, boxcar_snr_sweep<FUSED>, SW_THREADS, lay.total)) != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorInvalidConfiguration;
+    const int64_t wave = (int64_t)sms * per_sm;                 // persistent: one resident wave walks all tiles
+    const unsigned grid = (unsigned)(tiles < wave ? tiles : wave);
+    boxcar_snr_sweep<FUSED><<<grid, SW_THREADS, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax,
+                                                               snr, width, threshold, out, capacity, d_count);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
@@ -253,23 +370,9 @@ cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
                          bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
                          unsigned long long *d_count, cudaStream_t s)
 {
-    const int tpr = (int)((n_t + SW_TILE - 1) / SW_TILE);
-    const int64_t blocks = n_dm * (int64_t)tpr;
-    if (blocks > 2147483647LL) return cudaErrorInvalidConfiguration;
-    const size_t smem = (size_t)((zpad(sw_len(nmax)) + 1) & ~1) * sizeof(float2) + (size_t)sw_rt_len(nmax) * sizeof(float2);
-    cudaError_t e;
-    if (fused) {
-        e = cudaFuncSetAttribute(boxcar_snr_sweep<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        boxcar_snr_sweep<true><<<(unsigned)blocks, SW_THREADS, smem, s>>>(x, n_t, row_stride, tpr, d_stats, d_table, nmax,
-                                                                         nullptr, nullptr, threshold, out, capacity, d_count);
-    } else {
-        e = cudaFuncSetAttribute(boxcar_snr_sweep<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        boxcar_snr_sweep<false><<<(unsigned)blocks, SW_THREADS, smem, s>>>(x, n_t, row_stride, tpr, d_stats, d_table, nmax,
-                                                                          snr, width, 0.0f, nullptr, 0, nullptr);
-    }
-    return cudaGetLastError();
+    if (fused)
+        return launch_sweep_t<true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, nullptr, nullptr, threshold, out, capacity, d_count, s);
+    return launch_sweep_t<false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, 0.0f, nullptr, 0, nullptr, s);
 }
 
 }  // namespace spd
