@@ -10,14 +10,18 @@
 //    subtract, mu = mu_hi + mu_lo), so the inner loop is B += y; s = B * r_N with r_N = 1/sigma_N from a table.
 //  * One tile = 2048 consecutive samples of one row, as two sub-tiles A = [T0, T0+1024), B = [T0+1024, T0+2048).
 //    The working layout INTERLEAVES them, float2 Z[i] = (yA[i], yB[i]), so that one packed FADD2 / FMUL2
-//    (Blackwell packed fp32) advances one running sum of each sub-tile: the FMA pipe sees 2 lane-ops per
-//    (sample, width) pair -- the arithmetic floor -- for one issue slot per pair.
+//    (Blackwell packed fp32) advances one running sum of each sub-tile.  Measured on B200: a
+//    packed op holds the FMA pipe for two cycles but takes ONE issue slot, so the 3-input FMNMX of the running
+//    maximum and the arg-max bookkeeping (ALU pipe) issue in its shadow: the loop runs at the FMA-pipe floor of two
+//    lane-cycles per (sample, width) pair instead of the three issue slots of the scalar add / mul / max form.
 //  * Each thread owns 8 consecutive samples of each sub-tile and keeps a sliding window of 8 float2 in registers
 //    (the width loop is unrolled by 8, so the rotation is register renaming): one LDS.64 per width step.
 //  * Samples past the row end are staged as -inf: a running sum that has touched one is -inf for every wider
-//    width, so "only widths that fit" (reading A9) needs no masking in the loop.
-//  * arg-max is deferred: the running maximum is advanced with 3-input FMNMX only; per block of 8 widths one
-//    compare + one select record the block that last raised it.  After the loop that block alone is evaluated
+//    width, so "only widths that fit" (reading A9) needs no masking in the loop.  Widths nmax < w <= 8 ceil(nmax/8)
+//    get a NaN reciprocal: FMNMX drops NaN operands, so they can never win and need no tail loop.
+//  * arg-max is deferred: the running maximum is advanced with 3-input FMNMX only, ping-ponging between two
+//    register sets so that the value before and after each block of 8 widths are both live; one compare + one
+//    select per block then record the block that last raised it.  After the loop that block alone is evaluated
 //    again, width by width, from a tile-local prefix sum P kept in shared memory (B_w(t) = P[t+w] - P[t], no
 //    dependency chain), and the smallest width attaining the block maximum is taken.  Blocks ascend and every
 //    comparison is a strict '>', so ties keep the smallest width (A7).  The SNR written is the running-sum value
@@ -36,24 +40,23 @@ constexpr int SW_SUB     = SW_THREADS * SW_R;        // 1024
 constexpr int SW_TILE    = 2 * SW_SUB;               // 2048 samples per tile
 
 __host__ __device__ inline int zpad(int i) { return i + (i >> 3); }          // one pad float2 per 8: lane stride 72 B
-__host__ __device__ inline int sw_halo(int nmax) { return round_up(nmax, 8) + 24; }
-__host__ __device__ inline int sw_rt_len(int nmax) { return round_up(nmax, 8) + 24; }
+__host__ __device__ inline int sw_nblk(int nmax) { return (nmax + 7) >> 3; }  // blocks of 8 widths
+__host__ __device__ inline int sw_halo(int nmax) { return 8 * sw_nblk(nmax) + 8; }   // positions staged past a sub-tile
+__host__ __device__ inline int sw_rt_len(int nmax) { return 8 * sw_nblk(nmax) + 8; } // reciprocal-table entries
 
 size_t sweep_table_bytes(int nmax) { return (size_t)sw_rt_len(nmax) * sizeof(float); }
 
 struct SweepSmem {           // byte offsets into dynamic shared memory (all 16-byte aligned)
-    int z, raw, pa, pb, scan, rt2, rtf, total;
+    int z, raw, p2, scan, rt2, rtf, total;
     __host__ __device__ explicit SweepSmem(int nmax)
     {
         const int H = sw_halo(nmax), R = sw_rt_len(nmax);
-        const int P = round_up((zpad(SW_SUB + H + 1) + 1) * 4, 16);      // one prefix array (floats, zpad layout)
-        z = 0;
-        raw = z + round_up((zpad(SW_SUB + H) + 1) * 8, 16);
-        pa = raw + round_up((SW_TILE + H) * 4, 16);
-        pb = pa + P;
-        scan = pb + P;
-        rt2 = scan + 64;
-        rtf = rt2 + R * 8;
+        z = 0;                                                           // float2 Z[zpad(SUB + H)]
+        raw = z + round_up((zpad(SW_SUB + H) + 1) * 8, 16);              // float raw[TILE + H]
+        p2 = raw + round_up((SW_TILE + H) * 4, 16);                      // float2 P[zpad(SUB + H + 1)]: prefix sums
+        scan = p2 + round_up((zpad(SW_SUB + H + 1) + 1) * 8, 16);        // float2 [2][4]: per-warp totals of the scan
+        rt2 = scan + 64;                                                 // float2 (r_w, r_w)
+        rtf = rt2 + R * 8;                                               // float r_w
         total = rtf + round_up(R * 4, 16);
     }
 };
@@ -77,7 +80,7 @@ __global__ void sigma_table_kernel(const spd_stats_t *__restrict__ st, int nmax,
     const double sigma = st->sigma, snm = st->sigma_nmax;
     const bool bad = (mode != SPD_SIGMA_SQRT) && (st->nmax_of_sigma != nmax);
     for (int w = 1 + blockIdx.x * blockDim.x + threadIdx.x; w <= sw_rt_len(nmax); w += gridDim.x * blockDim.x) {
-        float r = 0.0f;
+        float r = __int_as_float(0x7fc00000);      // widths past nmax (padding of the last block of 8) never win
         if (w <= nmax) {
             double s = sqrt((double)w) * sigma;
             if (mode == SPD_SIGMA_LINEAR && nmax > 1) s += (double)(w - 1) * snm / (double)(nmax - 1);
@@ -96,43 +99,46 @@ cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, f
     return cudaGetLastError();
 }
 
-// 8 width steps: advance the 8 packed running sums, scale, fold into the running maxima.
-// On entry W[v] = Z[i0 + a0 + v] (a0 = width offset of the first step); on exit the window has moved by 8.
-__device__ __forceinline__ void sweep8(float2 (&B)[SW_R], float2 (&W)[SW_R], float2 (&best)[SW_R],
+// One block of 8 width steps: advance the 8 packed running sums, scale, fold into the running maxima.
+// out[j] = max(in[j], the 8 SNRs of this block); `in` stays intact so that the caller can tell whether the block
+// raised the maximum.  On entry W[v] = Z[8 tid + a0 + v] (a0 = width offset of the first step); on exit the window
+// has moved by 8.  zp -> Z[8 (tid + kb + 1)] (the next 8 window elements), rp -> (r_w, r_w) of the block.
+__device__ __forceinline__ void sweep8(float2 (&B)[SW_R], float2 (&W)[SW_R], const float2 (&in)[SW_R], float2 (&out)[SW_R],
                                        const float2 *__restrict__ zp, const float2 *__restrict__ rp)
 {
 #pragma unroll
     for (int u = 0; u < 8; u += 2) {
         const float4 rr = *reinterpret_cast<const float4 *>(rp + u);
         const float2 r0 = make_float2(rr.x, rr.y), r1 = make_float2(rr.z, rr.w);
-        float2 s0[SW_R], s1[SW_R];
-#pragma unroll
-        for (int j = 0; j < SW_R; ++j) { B[j] = __fadd2_rn(B[j], W[(j + u) & 7]); s0[j] = __fmul2_rn(B[j], r0); }
-        W[u] = zp[u];
-#pragma unroll
-        for (int j = 0; j < SW_R; ++j) { B[j] = __fadd2_rn(B[j], W[(j + u + 1) & 7]); s1[j] = __fmul2_rn(B[j], r1); }
-        W[u + 1] = zp[u + 1];
+        const float2 n0 = zp[u], n1 = zp[u + 1];
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) {
-            best[j].x = fmax3(best[j].x, s0[j].x, s1[j].x);
-            best[j].y = fmax3(best[j].y, s0[j].y, s1[j].y);
+            B[j] = __fadd2_rn(B[j], W[(j + u) & 7]);
+            const float2 s0 = __fmul2_rn(B[j], r0);
+            B[j] = __fadd2_rn(B[j], (j == SW_R - 1) ? n0 : W[(j + u + 1) & 7]);
+            const float2 s1 = __fmul2_rn(B[j], r1);
+            const float2 m = (u == 0) ? in[j] : out[j];
+            out[j].x = fmax3(m.x, s0.x, s1.x);
+            out[j].y = fmax3(m.y, s0.y, s1.y);
         }
+        W[u] = n0;
+        W[u + 1] = n1;
     }
 }
 
 // record, per running sum, whether the block of widths that just ended raised the maximum
-__device__ __forceinline__ void note_block(const float2 (&best)[SW_R], const float2 (&old)[SW_R], int w0,
+__device__ __forceinline__ void note_block(const float2 (&now)[SW_R], const float2 (&old)[SW_R], int w0,
                                            int (&w0x)[SW_R], int (&w0y)[SW_R])
 {
 #pragma unroll
     for (int j = 0; j < SW_R; ++j) {
-        w0x[j] = (best[j].x > old[j].x) ? w0 : w0x[j];
-        w0y[j] = (best[j].y > old[j].y) ? w0 : w0y[j];
+        w0x[j] = (now[j].x > old[j].x) ? w0 : w0x[j];
+        w0y[j] = (now[j].y > old[j].y) ? w0 : w0y[j];
     }
 }
 
 template <bool FUSED>
-__global__ void __launch_bounds__(SW_THREADS, 3)
+__global__ void __launch_bounds__(SW_THREADS, 4)
 boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                  const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
                  float *__restrict__ snr, uint16_t *__restrict__ width,
@@ -143,22 +149,22 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
     const SweepSmem lay(nmax);
     float2 *Z   = reinterpret_cast<float2 *>(smem_raw + lay.z);
     float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
+    float2 *P2  = reinterpret_cast<float2 *>(smem_raw + lay.p2);      // prefix sums of y: (sub-tile A, sub-tile B), zpad layout
+    float2 *scan = reinterpret_cast<float2 *>(smem_raw + lay.scan);   // [2][4] per-warp totals of the tile prefix scan
     float2 *rt2 = reinterpret_cast<float2 *>(smem_raw + lay.rt2);     // (r_w, r_w): operand of FMUL2
     float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);      // r_w plain: LDS.128 in the width search
-    float  *PA  = reinterpret_cast<float *>(smem_raw + lay.pa);       // prefix sums of y, sub-tile A (zpad layout)
-    float  *PB  = reinterpret_cast<float *>(smem_raw + lay.pb);       // prefix sums of y, sub-tile B
-    float2 *scan = reinterpret_cast<float2 *>(smem_raw + lay.scan);   // per-warp totals of the tile prefix scan
 
     const int tid = threadIdx.x;
+    const int lane = tid & 31, wid = tid >> 5;
+    const int nblk = sw_nblk(nmax);
     const int H = sw_halo(nmax);
     const int LRAW = SW_TILE + H;                 // raw floats per tile: x[T0 .. T0 + 2048 + H)
-    const int LZ = SW_SUB + H;                    // interleaved positions
+    const int LZ = SW_SUB + H;                    // interleaved positions (a multiple of 8)
+    const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
     const double mu = st->mean;
     const float mu_hi = (float)mu, mu_lo = (float)(mu - (double)mu_hi);
+    const float2 mu_hi2 = make_float2(-mu_hi, -mu_hi), mu_lo2 = make_float2(-mu_lo, -mu_lo);
     const float NINF = __int_as_float(0xff800000);
-    const int nblk8 = nmax >> 3, rem = nmax & 7;
-    const int SEG = (LZ + SW_THREADS - 1) / SW_THREADS;       // consecutive positions per thread in the prefix scan
-    const int lane = tid & 31, wid = tid >> 5;
 
     for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) { float r = __ldg(table + w); rt2[w] = make_float2(r, r); rtf[w] = r; }
 
@@ -191,97 +197,108 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
         const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
         cp_async_commit_wait_all();
         __syncthreads();                           // raw tile landed; everyone is done with the previous Z / P
-        {
-            // y = x - mu into the interleaved layout, and the tile-local inclusive prefix sums of y (per sub-tile)
-            const int lo = tid * SEG, hi = min(lo + SEG, LZ);
-            float2 run = make_float2(0.f, 0.f);
-            for (int i = lo; i < hi; ++i) {
-                const float2 y = make_float2((raw[i] - mu_hi) - mu_lo, (raw[SW_SUB + i] - mu_hi) - mu_lo);
-                Z[zpad(i)] = y;
-                run = __fadd2_rn(run, y);
-                PA[zpad(i + 1)] = run.x; PB[zpad(i + 1)] = run.y;
-            }
-            float2 inc = run;                       // inclusive scan of the thread totals across the CTA
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const float ox = __shfl_up_sync(0xffffffffu, inc.x, d), oy = __shfl_up_sync(0xffffffffu, inc.y, d);
-                if (lane >= d) { inc.x += ox; inc.y += oy; }
-            }
-            if (lane == 31) scan[wid] = inc;
-            __syncthreads();
-            float2 off;                             // exclusive prefix inside the warp (no inc - run: -inf - -inf is NaN)
-            off.x = __shfl_up_sync(0xffffffffu, inc.x, 1); off.y = __shfl_up_sync(0xffffffffu, inc.y, 1);
-            if (lane == 0) off = make_float2(0.f, 0.f);
-            for (int w = 0; w < wid; ++w) { off.x += scan[w].x; off.y += scan[w].y; }
-            for (int i = lo; i < hi; ++i) { PA[zpad(i + 1)] += off.x; PB[zpad(i + 1)] += off.y; }
-            if (tid == 0) { PA[0] = 0.f; PB[0] = 0.f; }
+
+        // ---- y = x - mu into the interleaved layout (lane-consecutive: conflict-free) ---------------------------
+        for (int i = tid; i < LZ; i += SW_THREADS) {
+            float2 y = make_float2(raw[i], raw[SW_SUB + i]);
+            y = __fadd2_rn(__fadd2_rn(y, mu_hi2), mu_lo2);
+            Z[zpad(i)] = y;
         }
-        __syncthreads();                           // Z and P complete; raw is free again
+        __syncthreads();                           // Z complete; raw is free again
         if (tile + gridDim.x < total_tiles) prefetch(tile + gridDim.x);
 
-        // ---- per-thread state ----------------------------------------------------------------------------------
-        float2 B[SW_R], W[SW_R], best[SW_R];
+        // ---- per-thread state; the first window doubles as part 0 of the prefix scan -----------------------------
+        float2 B[SW_R], W[SW_R], bestA[SW_R], bestB[SW_R];
         int w0x[SW_R], w0y[SW_R];
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) {
             B[j] = make_float2(0.f, 0.f);
             W[j] = Z[9 * tid + j];                           // zpad(8 tid + j) = 9 tid + j
-            best[j] = make_float2(NINF, NINF);
+            bestA[j] = make_float2(NINF, NINF);
             w0x[j] = 0; w0y[j] = 0;
         }
 
-        // ---- main loop: one iteration = one block of 8 widths ------------------------------------------------------
-        for (int kb = 0; kb < nblk8; ++kb) {
-            float2 old[SW_R];
+        // ---- tile-local inclusive prefix sums P[i + 1] = y[0] + ... + y[i], per sub-tile (only the width search reads them)
+        {
+            float2 carry = make_float2(0.f, 0.f);
+            for (int part = 0; part < nparts; ++part) {
+                const int g = part * SW_THREADS + tid;           // group of 8 positions: 8 g .. 8 g + 7
+                const bool act = 8 * g < LZ;
+                float2 v[SW_R];
 #pragma unroll
-            for (int j = 0; j < SW_R; ++j) old[j] = best[j];
-            sweep8(B, W, best, Z + 9 * (tid + kb + 1), rt2 + 8 * kb);             // zpad(8 tid + 8 kb + 8 + u)
-            note_block(best, old, 8 * kb, w0x, w0y);
+                for (int j = 0; j < SW_R; ++j) v[j] = (part == 0) ? W[j] : (act ? Z[9 * g + j] : make_float2(0.f, 0.f));
+#pragma unroll
+                for (int j = 1; j < SW_R; ++j) v[j] = __fadd2_rn(v[j], v[j - 1]);
+                float2 inc = v[SW_R - 1];                        // inclusive scan of the thread totals across the warp
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const float ox = __shfl_up_sync(0xffffffffu, inc.x, d), oy = __shfl_up_sync(0xffffffffu, inc.y, d);
+                    if (lane >= d) { inc.x += ox; inc.y += oy; }
+                }
+                float2 *tot = scan + 4 * (part & 1);
+                if (lane == 31) tot[wid] = inc;
+                float2 off;                                      // exclusive prefix inside the warp (no inc - total: -inf - -inf is NaN)
+                off.x = __shfl_up_sync(0xffffffffu, inc.x, 1); off.y = __shfl_up_sync(0xffffffffu, inc.y, 1);
+                if (lane == 0) off = make_float2(0.f, 0.f);
+                __syncthreads();
+                off = __fadd2_rn(off, carry);
+#pragma unroll
+                for (int w = 0; w < SW_THREADS / 32; ++w) {
+                    const float2 t = tot[w];
+                    if (w < wid) off = __fadd2_rn(off, t);
+                    carry = __fadd2_rn(carry, t);
+                }
+                if (act) {
+#pragma unroll
+                    for (int j = 0; j < SW_R; ++j) P2[zpad(8 * g + j + 1)] = __fadd2_rn(v[j], off);
+                }
+            }
+            if (tid == 0) P2[0] = make_float2(0.f, 0.f);
         }
+        __syncthreads();                           // P complete
+
+        // ---- main loop: blocks of 8 widths, the running maximum ping-pongs between bestA and bestB ---------------------
+        {
+            const float2 *zp = Z + 9 * (tid + 1);                // zpad(8 tid + 8 kb + 8 + u) = 9 (tid + kb + 1) + u
+            const float2 *rp = rt2;
+            int kb = 0;
+            for (; kb + 2 <= nblk; kb += 2) {
+                sweep8(B, W, bestA, bestB, zp, rp);
+                note_block(bestB, bestA, 8 * kb, w0x, w0y);
+                sweep8(B, W, bestB, bestA, zp + 9, rp + 8);
+                note_block(bestA, bestB, 8 * kb + 8, w0x, w0y);
+                zp += 18; rp += 16;
+            }
+            if (kb < nblk) {
+                sweep8(B, W, bestA, bestB, zp, rp);
+                note_block(bestB, bestA, 8 * kb, w0x, w0y);
+#pragma unroll
+                for (int j = 0; j < SW_R; ++j) bestA[j] = bestB[j];
+            }
+        }
+        float2 (&best)[SW_R] = bestA;
 
         // ---- width search inside the winning block, from the prefix sums: B_w(t) = P[t + w] - P[t] ------------------
         int wx[SW_R], wy[SW_R];
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) {
-            wx[j] = 1; wy[j] = 1;
-            if (nblk8 > 0) {
+            const float2 p0 = P2[9 * tid + j];                                    // P[t], t = 8 tid + j
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int w0 = h ? w0y[j] : w0x[j];
-                    const float *Ph = h ? PB : PA;
-                    const float p0 = Ph[9 * tid + j];                             // P[t], t = 8 tid + j
-                    const float *pe = Ph + 9 * (tid + (w0 >> 3));                 // zpad(8 tid + w0 + c) = 9 (tid + w0/8) + c + (c >> 3)
-                    const float4 *rq = reinterpret_cast<const float4 *>(rtf + w0);
-                    const float4 ra = rq[0], rb = rq[1];
-                    const float r[8] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y, rb.z, rb.w};
-                    float s[8];
+            for (int h = 0; h < 2; ++h) {
+                const int w0 = h ? w0y[j] : w0x[j];
+                const float p0h = h ? p0.y : p0.x;
+                const float *pe = reinterpret_cast<const float *>(P2 + 9 * (tid + (w0 >> 3))) + h;   // zpad(8 tid + w0 + c) = 9 (tid + w0/8) + c + (c >> 3)
+                const float4 *rq = reinterpret_cast<const float4 *>(rtf + w0);
+                const float4 ra = rq[0], rb = rq[1];
+                const float r[8] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y, rb.z, rb.w};
+                float s[8];
 #pragma unroll
-                    for (int g = 0; g < 8; ++g) { const int c = j + g + 1; s[g] = (pe[c + (c >> 3)] - p0) * r[g]; }
-                    const float m = fmaxf(fmax3(fmax3(s[0], s[1], s[2]), s[3], s[4]), fmax3(s[5], s[6], s[7]));
-                    int w = 0;
+                for (int g = 0; g < 8; ++g) { const int c = j + g + 1; s[g] = (pe[2 * (c + (c >> 3))] - p0h) * r[g]; }
+                const float m = fmaxf(fmax3(fmax3(s[0], s[1], s[2]), s[3], s[4]), fmax3(s[5], s[6], s[7]));
+                int w = 0;
 #pragma unroll
-                    for (int g = 7; g >= 0; --g) w = (s[g] == m) ? g : w;
-                    if (h) wy[j] = w0 + w + 1; else wx[j] = w0 + w + 1;
-                }
-            }
-        }
-
-        // ---- tail widths (nmax not a multiple of 8): per-width tracking; wider widths, so strict '>' is still right
-        if (rem) {
-            const float2 *zp = Z + 9 * (tid + nblk8 + 1);
-            for (int u = 0; u < rem; ++u) {
-                const float2 r = rt2[8 * nblk8 + u];
-                const int wv = 8 * nblk8 + u + 1;
-#pragma unroll
-                for (int j = 0; j < SW_R; ++j) {
-                    B[j] = __fadd2_rn(B[j], W[j]);
-                    const float2 s = __fmul2_rn(B[j], r);
-                    if (s.x > best[j].x) { best[j].x = s.x; wx[j] = wv; }
-                    if (s.y > best[j].y) { best[j].y = s.y; wy[j] = wv; }
-                }
-#pragma unroll
-                for (int j = 0; j < SW_R - 1; ++j) W[j] = W[j + 1];  // rem < 8 steps: a plain shift is fine here
-                W[SW_R - 1] = zp[u];
+                for (int g = 7; g >= 0; --g) w = (s[g] == m) ? g : w;
+                if (h) wy[j] = w0 + w + 1; else wx[j] = w0 + w + 1;
             }
         }
 
