@@ -28,6 +28,7 @@ import gen  # noqa: E402
 
 METRIC = "DM×time samples/s through boxcar SNR search (×real-time); HBM GB/s vs peak"
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
+OPS_PER_PAIR = 3.0      # fp32 add + fp32 multiply + compare per (sample, width) pair
 # DRAM bytes per launch of boxcar_snr_sweep on config 3 from `ncu --set full` (profiles/r01_sweep_full.md); None = not captured
 SWEEP_DRAM_TRAFFIC_C3 = None
 
@@ -260,19 +261,22 @@ def run_ours(args):
         hbm_peak, sm_max_mhz, peak_kind = _peaks()
         pairs = float(n) * nmax
         sweep_ms = float(np.mean(t_sweep))
-        alu_peak = SM_COUNT * FP32_LANES_PER_SM * sm_max_mhz * 1e6 / 1e12          # T lane-instructions/s
-        alu_ach = 2.0 * pairs / (sweep_ms * 1e-3) / 1e12                            # one fp32 add + one fp32 multiply per pair
+        # FP32 roofline of the sweep: one fp32 add, one fp32 multiply and one compare per (sample, width)
+        # pair = 3 lane-ops; peak = one 32-lane instruction per SM sub-partition per clock = 148 x 128 lanes x sm_max_mhz.
+        alu_peak = SM_COUNT * FP32_LANES_PER_SM * sm_max_mhz * 1e6 / 1e12          # T lane-ops/s
+        alu_ach = OPS_PER_PAIR * pairs / (sweep_ms * 1e-3) / 1e12
         hbm_ach = 10.0 * n / (sweep_ms * 1e-3) / 1e9
-        hbm_bound = (10.0 * n / (hbm_peak * 1e9)) > (2.0 * pairs / (alu_peak * 1e12))
+        hbm_bound = (10.0 * n / (hbm_peak * 1e9)) > (OPS_PER_PAIR * pairs / (alu_peak * 1e12))
         roof = ({"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak}
                 if hbm_bound else
                 {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": alu_ach / alu_peak})
         roof.update({"kernel": "boxcar_snr_sweep", "traffic": SWEEP_DRAM_TRAFFIC_C3 if (cfg.cid % 100 == 3 and nmax == 128 and n_dm == 6000) else None,
                      "peak_source": f"{peak_kind} (MEASURED_PEAKS.json)" if roof["bound"] == "hbm" else
-                                    "derived: 148 SM x 128 fp32 lanes x sm_max_mhz (FMA pipe, non-fused ops); 2 flops (add, multiply) per (sample,width) pair",
-                     "ms_per_launch": sweep_ms, "algorithmic_bytes_per_sample": 10, "flops_per_pair": 2,
+                                    "derived (DESIGN.md section 7): 148 SM x 128 fp32 lanes x sm_max_mhz; 3 lane-ops (add, multiply, compare) per (sample,width) pair",
+                     "ms_per_launch": sweep_ms, "algorithmic_bytes_per_sample": 10, "ops_per_pair": OPS_PER_PAIR,
                      "hbm_GBps": hbm_ach, "hbm_frac_of_measured": hbm_ach / hbm_peak, "hbm_frac_of_8TBps": hbm_ach / 8000.0,
-                     "alu_Tops": alu_ach, "alu_frac": alu_ach / alu_peak})
+                     "alu_Tops": alu_ach, "alu_frac": alu_ach / alu_peak,
+                     "alu_frac_add_mul_only": 2.0 * pairs / (sweep_ms * 1e-3) / 1e12 / alu_peak})
         cpu = None
         if not args.no_cpu_baseline:
             v, cores, sample, _ = oracle_sample_rate(gen.get_config(args.config), nmax, args.cpu_seconds)
