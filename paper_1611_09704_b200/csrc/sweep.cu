@@ -198,35 +198,44 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
         cp_async_commit_wait_all();
         __syncthreads();                           // raw tile landed; everyone is done with the previous Z / P
 
-        // ---- y = x - mu into the interleaved layout (lane-consecutive: conflict-free) ---------------------------
-        for (int i = tid; i < LZ; i += SW_THREADS) {
-            float2 y = make_float2(raw[i], raw[SW_SUB + i]);
-            y = __fadd2_rn(__fadd2_rn(y, mu_hi2), mu_lo2);
-            Z[zpad(i)] = y;
-        }
-        __syncthreads();                           // Z complete; raw is free again
-        if (tile + gridDim.x < total_tiles) prefetch(tile + gridDim.x);
-
-        // ---- per-thread state; the first window doubles as part 0 of the prefix scan -----------------------------
+        // ---- per-thread state ---------------------------------------------------------------------------------------
         float2 B[SW_R], W[SW_R], bestA[SW_R], bestB[SW_R];
         int w0x[SW_R], w0y[SW_R];
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) {
             B[j] = make_float2(0.f, 0.f);
-            W[j] = Z[9 * tid + j];                           // zpad(8 tid + j) = 9 tid + j
             bestA[j] = make_float2(NINF, NINF);
             w0x[j] = 0; w0y[j] = 0;
         }
 
-        // ---- tile-local inclusive prefix sums P[i + 1] = y[0] + ... + y[i], per sub-tile (only the width search reads them)
+        // ---- staging, one pass: every thread takes groups of 8 consecutive positions (part 0: its own 8 samples, whose
+        //      y values stay in registers as the first window), forms y = x - mu (two-term fp32 subtract), writes the
+        //      interleaved Z and the tile-local inclusive prefix sums P[i + 1] = y[0] + ... + y[i] of both sub-tiles
+        //      (only the width search reads P)
         {
             float2 carry = make_float2(0.f, 0.f);
             for (int part = 0; part < nparts; ++part) {
                 const int g = part * SW_THREADS + tid;           // group of 8 positions: 8 g .. 8 g + 7
                 const bool act = 8 * g < LZ;
                 float2 v[SW_R];
+                if (act) {
+                    const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
+                    const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
+                    v[0] = make_float2(a0.x, b0.x); v[1] = make_float2(a0.y, b0.y); v[2] = make_float2(a0.z, b0.z); v[3] = make_float2(a0.w, b0.w);
+                    v[4] = make_float2(a1.x, b1.x); v[5] = make_float2(a1.y, b1.y); v[6] = make_float2(a1.z, b1.z); v[7] = make_float2(a1.w, b1.w);
 #pragma unroll
-                for (int j = 0; j < SW_R; ++j) v[j] = (part == 0) ? W[j] : (act ? Z[9 * g + j] : make_float2(0.f, 0.f));
+                    for (int j = 0; j < SW_R; ++j) {
+                        v[j] = __fadd2_rn(__fadd2_rn(v[j], mu_hi2), mu_lo2);
+                        Z[9 * g + j] = v[j];                     // zpad(8 g + j) = 9 g + j
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < SW_R; ++j) v[j] = make_float2(0.f, 0.f);
+                }
+                if (part == 0) {
+#pragma unroll
+                    for (int j = 0; j < SW_R; ++j) W[j] = v[j];
+                }
 #pragma unroll
                 for (int j = 1; j < SW_R; ++j) v[j] = __fadd2_rn(v[j], v[j - 1]);
                 float2 inc = v[SW_R - 1];                        // inclusive scan of the thread totals across the warp
@@ -240,7 +249,8 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
                 float2 off;                                      // exclusive prefix inside the warp (no inc - total: -inf - -inf is NaN)
                 off.x = __shfl_up_sync(0xffffffffu, inc.x, 1); off.y = __shfl_up_sync(0xffffffffu, inc.y, 1);
                 if (lane == 0) off = make_float2(0.f, 0.f);
-                __syncthreads();
+                __syncthreads();                                 // totals visible; this part of raw is consumed, of Z written
+                if (part == nparts - 1 && tile + gridDim.x < total_tiles) prefetch(tile + gridDim.x);   // raw is free again
                 off = __fadd2_rn(off, carry);
 #pragma unroll
                 for (int w = 0; w < SW_THREADS / 32; ++w) {

@@ -46,7 +46,7 @@ def test_two_row_blocks_merged_equal_the_whole_chunk(P, mode, nmax):
     a, b = P.read_stats(st)[0], P.read_stats(st_all)[0]
     assert a["n"] == b["n"] and a["n_b"] == b["n_b"]
     for k in ("mean", "sigma") + (("sigma_nmax",) if mode != "sqrt" else ()):
-        assert abs(a[k] - b[k]) <= 1e-9 * max(abs(b[k]), b["sigma"])
+        assert abs(a[k] - b[k]) <= 1e-7 * max(abs(b[k]), b["sigma"])      # fp32 warp chunks are shifted by a per-call K: not bit-equal
     recs = []
     for lo, d in blocks:
         out, cnt = P.spd_search_fused(d, st_all, nmax, mode, cfg.threshold, capacity=1 << 16)   # same statistics => identical records
