@@ -99,6 +99,30 @@ cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, f
     return cudaGetLastError();
 }
 
+// raw tile -> shared memory, asynchronously where the 16-byte fast path applies; past the row end -> -inf
+__device__ __forceinline__ void stage_tile(float *__restrict__ raw, const float *__restrict__ x, int64_t n_t, int64_t row_stride,
+                                           int tiles_per_row, int64_t tile, int LRAW, int tid)
+{
+    const float NINF = __int_as_float(0xff800000);
+    const int64_t row = tile / tiles_per_row;
+    const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
+    const float *rowp = x + row * row_stride;
+    const bool vec = ((reinterpret_cast<uintptr_t>(rowp) & 15) == 0);
+    if (vec && T0 + LRAW <= n_t) {                       // interior tile: no bounds checks
+        const float *src = rowp + T0;
+        for (int p = tid; p < LRAW / 4; p += SW_THREADS) cp_async16(raw + 4 * p, src + 4 * p);
+    } else {
+        for (int p = tid; p < LRAW / 4; p += SW_THREADS) {
+            const int64_t pos = T0 + 4 * p;
+            if (vec && pos + 3 < n_t) cp_async16(raw + 4 * p, rowp + pos);
+            else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) raw[4 * p + k] = (pos + k < n_t) ? __ldg(rowp + pos + k) : NINF;
+            }
+        }
+    }
+}
+
 // One block of 8 width steps: advance the 8 packed running sums, scale, fold into the running maxima.
 // out[j] = max(in[j], the 8 SNRs of this block); `in` stays intact so that the caller can tell whether the block
 // raised the maximum.  On entry W[v] = Z[8 tid + a0 + v] (a0 = width offset of the first step); on exit the window
@@ -137,13 +161,10 @@ __device__ __forceinline__ void note_block(const float2 (&now)[SW_R], const floa
     }
 }
 
-template <bool FUSED>
 __global__ void __launch_bounds__(SW_THREADS, 4)
 boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                  const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
-                 float *__restrict__ snr, uint16_t *__restrict__ width,
-                 float threshold, spd_candidate_t *__restrict__ cand, unsigned long long capacity,
-                 unsigned long long *__restrict__ count)
+                 float *__restrict__ snr, uint16_t *__restrict__ width)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const SweepSmem lay(nmax);
@@ -168,26 +189,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
 
     for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) { float r = __ldg(table + w); rt2[w] = make_float2(r, r); rtf[w] = r; }
 
-    // raw tile -> shared memory, asynchronously where the 16-byte fast path applies; past the row end -> -inf
-    auto prefetch = [&](int64_t tile) {
-        const int64_t row = tile / tiles_per_row;
-        const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
-        const float *rowp = x + row * row_stride;
-        const bool vec = ((reinterpret_cast<uintptr_t>(rowp) & 15) == 0);
-        if (vec && T0 + LRAW <= n_t) {                       // interior tile: no bounds checks
-            const float *src = rowp + T0;
-            for (int p = tid; p < LRAW / 4; p += SW_THREADS) cp_async16(raw + 4 * p, src + 4 * p);
-        } else {
-            for (int p = tid; p < LRAW / 4; p += SW_THREADS) {
-                const int64_t pos = T0 + 4 * p;
-                if (vec && pos + 3 < n_t) cp_async16(raw + 4 * p, rowp + pos);
-                else {
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) raw[4 * p + k] = (pos + k < n_t) ? __ldg(rowp + pos + k) : NINF;
-                }
-            }
-        }
-    };
+    auto prefetch = [&](int64_t tile) { stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile, LRAW, tid); };
 
     int64_t tile = blockIdx.x;
     if (tile < total_tiles) prefetch(tile);
@@ -320,76 +322,168 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
 
         // ---- results ----------------------------------------------------------------------------------------------
         const int64_t ta = T0 + SW_R * tid, tb = ta + SW_SUB;
-        if (!FUSED) {
-            float *oa = snr + row * row_stride + ta, *ob = snr + row * row_stride + tb;
-            const bool v4 = ((reinterpret_cast<uintptr_t>(snr + row * row_stride) & 15) == 0);
-            if (v4 && ta + 7 < n_t) {
-                __stcs(reinterpret_cast<float4 *>(oa), make_float4(best[0].x, best[1].x, best[2].x, best[3].x));
-                __stcs(reinterpret_cast<float4 *>(oa) + 1, make_float4(best[4].x, best[5].x, best[6].x, best[7].x));
-            } else {
-#pragma unroll
-                for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) oa[j] = best[j].x;
-            }
-            if (v4 && tb + 7 < n_t) {
-                __stcs(reinterpret_cast<float4 *>(ob), make_float4(best[0].y, best[1].y, best[2].y, best[3].y));
-                __stcs(reinterpret_cast<float4 *>(ob) + 1, make_float4(best[4].y, best[5].y, best[6].y, best[7].y));
-            } else {
-#pragma unroll
-                for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) ob[j] = best[j].y;
-            }
-            if (width) {
-                uint16_t *wa = width + row * row_stride + ta, *wb = width + row * row_stride + tb;
-                const bool w8 = ((reinterpret_cast<uintptr_t>(width + row * row_stride) & 15) == 0);
-                if (w8 && ta + 7 < n_t)
-                    __stcs(reinterpret_cast<uint4 *>(wa), make_uint4(wx[0] | (wx[1] << 16), wx[2] | (wx[3] << 16), wx[4] | (wx[5] << 16), wx[6] | (wx[7] << 16)));
-                else {
-#pragma unroll
-                    for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) wa[j] = (uint16_t)wx[j];
-                }
-                if (w8 && tb + 7 < n_t)
-                    __stcs(reinterpret_cast<uint4 *>(wb), make_uint4(wy[0] | (wy[1] << 16), wy[2] | (wy[3] << 16), wy[4] | (wy[5] << 16), wy[6] | (wy[7] << 16)));
-                else {
-#pragma unroll
-                    for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) wb[j] = (uint16_t)wy[j];
-                }
-            }
+        float *oa = snr + row * row_stride + ta, *ob = snr + row * row_stride + tb;
+        const bool v4 = ((reinterpret_cast<uintptr_t>(snr + row * row_stride) & 15) == 0);
+        if (v4 && ta + 7 < n_t) {
+            __stcs(reinterpret_cast<float4 *>(oa), make_float4(best[0].x, best[1].x, best[2].x, best[3].x));
+            __stcs(reinterpret_cast<float4 *>(oa) + 1, make_float4(best[4].x, best[5].x, best[6].x, best[7].x));
         } else {
-            // threshold in the same kernel: planes are never written
-            bool any = false;
 #pragma unroll
-            for (int j = 0; j < SW_R; ++j) any |= (best[j].x >= threshold && ta + j < n_t) || (best[j].y >= threshold && tb + j < n_t);
-            if (__any_sync(0xffffffffu, any)) {
+            for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) oa[j] = best[j].x;
+        }
+        if (v4 && tb + 7 < n_t) {
+            __stcs(reinterpret_cast<float4 *>(ob), make_float4(best[0].y, best[1].y, best[2].y, best[3].y));
+            __stcs(reinterpret_cast<float4 *>(ob) + 1, make_float4(best[4].y, best[5].y, best[6].y, best[7].y));
+        } else {
 #pragma unroll
-                for (int j = 0; j < SW_R; ++j) {
-                    append_candidate(best[j].x >= threshold && ta + j < n_t, (uint32_t)row, (uint32_t)(ta + j), best[j].x, (uint32_t)wx[j], cand, capacity, count);
-                    append_candidate(best[j].y >= threshold && tb + j < n_t, (uint32_t)row, (uint32_t)(tb + j), best[j].y, (uint32_t)wy[j], cand, capacity, count);
-                }
+            for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) ob[j] = best[j].y;
+        }
+        if (width) {
+            uint16_t *wa = width + row * row_stride + ta, *wb = width + row * row_stride + tb;
+            const bool w8 = ((reinterpret_cast<uintptr_t>(width + row * row_stride) & 15) == 0);
+            if (w8 && ta + 7 < n_t)
+                __stcs(reinterpret_cast<uint4 *>(wa), make_uint4(wx[0] | (wx[1] << 16), wx[2] | (wx[3] << 16), wx[4] | (wx[5] << 16), wx[6] | (wx[7] << 16)));
+            else {
+#pragma unroll
+                for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) wa[j] = (uint16_t)wx[j];
+            }
+            if (w8 && tb + 7 < n_t)
+                __stcs(reinterpret_cast<uint4 *>(wb), make_uint4(wy[0] | (wy[1] << 16), wy[2] | (wy[3] << 16), wy[4] | (wy[5] << 16), wy[6] | (wy[7] << 16)));
+            else {
+#pragma unroll
+                for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) wb[j] = (uint16_t)wy[j];
             }
         }
     }
     cp_async_commit_wait_all();
 }
 
-template <bool FUSED>
-static cudaError_t launch_sweep_t(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
-                                  const float *d_table, int nmax, float *snr, uint16_t *width, float threshold,
-                                  spd_candidate_t *out, unsigned long long capacity, unsigned long long *d_count, cudaStream_t s)
+// ---------------------------------------------------------------------------------------------------------------
+// Fused search (spd_search_fused): the same width loop with the threshold of PAPER.md:87-93 applied in
+// the kernel.  The planes are never written, so the width is needed at hits only: there is no per-block arg-max
+// bookkeeping, no prefix scan and no width search.  A thread that owns a hit replays that one sample's running sums
+// in the order of the main loop (same fp32 adds and multiplies, so the values are bit-identical) and takes the first
+// width whose SNR equals the maximum: the smallest arg-max (A7).
+struct FusedSmem {
+    int z, raw, rt2, rtf, total;
+    __host__ __device__ explicit FusedSmem(int nmax)
+    {
+        const int H = sw_halo(nmax), R = sw_rt_len(nmax);
+        z = 0;
+        raw = z + round_up((zpad(SW_SUB + H) + 1) * 8, 16);
+        rt2 = raw + round_up((SW_TILE + H) * 4, 16);
+        rtf = rt2 + R * 8;
+        total = rtf + round_up(R * 4, 16);
+    }
+};
+
+__device__ __noinline__ int replay_width(const float *__restrict__ zh, int pos, const float *__restrict__ rtf, int nmax, float best)
 {
-    const int tpr = (int)((n_t + SW_TILE - 1) / SW_TILE);
-    const int64_t tiles = n_dm * (int64_t)tpr;
-    const SweepSmem lay(nmax);
-    cudaError_t e = cudaFuncSetAttribute(boxcar_snr_sweep<FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, lay.total);
+    float b = 0.f;
+    for (int w = 1; w <= nmax; ++w) {
+        b = __fadd_rn(b, zh[2 * zpad(pos + w - 1)]);
+        if (__fmul_rn(b, rtf[w - 1]) == best) return w;
+    }
+    return nmax;                                   // not reached for finite input
+}
+
+__global__ void __launch_bounds__(SW_THREADS, 5)
+boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
+                    const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
+                    float threshold, spd_candidate_t *__restrict__ cand, unsigned long long capacity,
+                    unsigned long long *__restrict__ count)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const FusedSmem lay(nmax);
+    float2 *Z   = reinterpret_cast<float2 *>(smem_raw + lay.z);
+    float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
+    float2 *rt2 = reinterpret_cast<float2 *>(smem_raw + lay.rt2);
+    float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);
+
+    const int tid = threadIdx.x;
+    const int nblk = sw_nblk(nmax);
+    const int H = sw_halo(nmax);
+    const int LRAW = SW_TILE + H, LZ = SW_SUB + H;
+    const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
+    const double mu = st->mean;
+    const float mu_hi = (float)mu, mu_lo = (float)(mu - (double)mu_hi);
+    const float2 mu_hi2 = make_float2(-mu_hi, -mu_hi), mu_lo2 = make_float2(-mu_lo, -mu_lo);
+    const float NINF = __int_as_float(0xff800000);
+
+    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) { float r = __ldg(table + w); rt2[w] = make_float2(r, r); rtf[w] = r; }
+
+    int64_t tile = blockIdx.x;
+    if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile, LRAW, tid);
+
+    for (; tile < total_tiles; tile += gridDim.x) {
+        const int64_t row = tile / tiles_per_row;
+        const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
+        cp_async_commit_wait_all();
+        __syncthreads();                           // raw tile landed; everyone is done with the previous Z
+
+        float2 B[SW_R], W[SW_R], best[SW_R];
+        for (int part = 0; part < nparts; ++part) {
+            const int g = part * SW_THREADS + tid;
+            if (8 * g < LZ) {
+                const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
+                const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
+                float2 v[SW_R] = {make_float2(a0.x, b0.x), make_float2(a0.y, b0.y), make_float2(a0.z, b0.z), make_float2(a0.w, b0.w),
+                                  make_float2(a1.x, b1.x), make_float2(a1.y, b1.y), make_float2(a1.z, b1.z), make_float2(a1.w, b1.w)};
+#pragma unroll
+                for (int j = 0; j < SW_R; ++j) {
+                    v[j] = __fadd2_rn(__fadd2_rn(v[j], mu_hi2), mu_lo2);
+                    Z[9 * g + j] = v[j];
+                    if (part == 0) W[j] = v[j];
+                }
+            }
+        }
+        __syncthreads();                           // Z complete; raw is free again
+        if (tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile + gridDim.x, LRAW, tid);
+
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); }
+        {
+            const float2 *zp = Z + 9 * (tid + 1);
+            const float2 *rp = rt2;
+            for (int kb = 0; kb < nblk; ++kb, zp += 9, rp += 8) sweep8(B, W, best, best, zp, rp);
+        }
+
+        // ---- threshold; hits replay their own running sums to get the width ------------------------------------------
+        const int64_t ta = T0 + SW_R * tid, tb = ta + SW_SUB;
+        bool any = false;
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) any |= (best[j].x >= threshold && ta + j < n_t) || (best[j].y >= threshold && tb + j < n_t);
+        if (__any_sync(0xffffffffu, any)) {
+            const float *zf = reinterpret_cast<const float *>(Z);
+#pragma unroll
+            for (int j = 0; j < SW_R; ++j) {
+                const bool ha = best[j].x >= threshold && ta + j < n_t;
+                const bool hb = best[j].y >= threshold && tb + j < n_t;
+                int wa = 1, wb = 1;
+                if (ha) wa = replay_width(zf, SW_R * tid + j, rtf, nmax, best[j].x);
+                if (hb) wb = replay_width(zf + 1, SW_R * tid + j, rtf, nmax, best[j].y);
+                __syncwarp();
+                append_candidate(ha, (uint32_t)row, (uint32_t)(ta + j), best[j].x, (uint32_t)wa, cand, capacity, count);
+                append_candidate(hb, (uint32_t)row, (uint32_t)(tb + j), best[j].y, (uint32_t)wb, cand, capacity, count);
+            }
+        }
+    }
+    cp_async_commit_wait_all();
+}
+
+template <typename K>
+static cudaError_t persistent_grid(K kernel, int smem, int64_t tiles, unsigned *grid)
+{
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 0, per_sm = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, boxcar_snr_sweep<FUSED>, SW_THREADS, lay.total)) != cudaSuccess) return e;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, SW_THREADS, smem)) != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorInvalidConfiguration;
     const int64_t wave = (int64_t)sms * per_sm;                 // persistent: one resident wave walks all tiles
-    const unsigned grid = (unsigned)(tiles < wave ? tiles : wave);
-    boxcar_snr_sweep<FUSED><<<grid, SW_THREADS, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax,
-                                                               snr, width, threshold, out, capacity, d_count);
-    return cudaGetLastError();
+    *grid = (unsigned)(tiles < wave ? tiles : wave);
+    return cudaSuccess;
 }
 
 cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
@@ -397,9 +491,21 @@ cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
                          bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
                          unsigned long long *d_count, cudaStream_t s)
 {
-    if (fused)
-        return launch_sweep_t<true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, nullptr, nullptr, threshold, out, capacity, d_count, s);
-    return launch_sweep_t<false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, 0.0f, nullptr, 0, nullptr, s);
+    const int tpr = (int)((n_t + SW_TILE - 1) / SW_TILE);
+    const int64_t tiles = n_dm * (int64_t)tpr;
+    unsigned grid = 0;
+    cudaError_t e;
+    if (fused) {
+        const FusedSmem lay(nmax);
+        if ((e = persistent_grid(boxcar_search_fused, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_search_fused<<<grid, SW_THREADS, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax,
+                                                                threshold, out, capacity, d_count);
+    } else {
+        const SweepSmem lay(nmax);
+        if ((e = persistent_grid(boxcar_snr_sweep, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep<<<grid, SW_THREADS, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
+    }
+    return cudaGetLastError();
 }
 
 }  // namespace spd
