@@ -47,7 +47,7 @@ __host__ __device__ inline int sw_rt_len(int nmax) { return 8 * sw_nblk(nmax) + 
 size_t sweep_table_bytes(int nmax) { return (size_t)sw_rt_len(nmax) * sizeof(float); }
 
 struct SweepSmem {           // byte offsets into dynamic shared memory (all 16-byte aligned)
-    int z, raw, p2, scan, rt2, rtf, total;
+    int z, raw, p2, scan, rtf, total;
     __host__ __device__ explicit SweepSmem(int nmax)
     {
         const int H = sw_halo(nmax), R = sw_rt_len(nmax);
@@ -55,8 +55,7 @@ struct SweepSmem {           // byte offsets into dynamic shared memory (all 16-
         raw = z + round_up((zpad(SW_SUB + H) + 1) * 8, 16);              // float raw[TILE + H]
         p2 = raw + round_up((SW_TILE + H) * 4, 16);                      // float2 P[zpad(SUB + H + 1)]: prefix sums
         scan = p2 + round_up((zpad(SW_SUB + H + 1) + 1) * 8, 16);        // float2 [2][4]: per-warp totals of the scan
-        rt2 = scan + 64;                                                 // float2 (r_w, r_w)
-        rtf = rt2 + R * 8;                                               // float r_w
+        rtf = scan + 64;                                                 // float r_w
         total = rtf + round_up(R * 4, 16);
     }
 };
@@ -126,14 +125,15 @@ __device__ __forceinline__ void stage_tile(float *__restrict__ raw, const float 
 // One block of 8 width steps: advance the 8 packed running sums, scale, fold into the running maxima.
 // out[j] = max(in[j], the 8 SNRs of this block); `in` stays intact so that the caller can tell whether the block
 // raised the maximum.  On entry W[v] = Z[8 tid + a0 + v] (a0 = width offset of the first step); on exit the window
-// has moved by 8.  zp -> Z[8 (tid + kb + 1)] (the next 8 window elements), rp -> (r_w, r_w) of the block.
+// has moved by 8.  zp -> Z[8 (tid + kb + 1)] (the next 8 window elements), rp -> r_w of the block (a scalar operand:
+// FMUL2 broadcasts one register to both halves, which costs one register read less than a (r_w, r_w) pair).
 __device__ __forceinline__ void sweep8(float2 (&B)[SW_R], float2 (&W)[SW_R], const float2 (&in)[SW_R], float2 (&out)[SW_R],
-                                       const float2 *__restrict__ zp, const float2 *__restrict__ rp)
+                                       const float2 *__restrict__ zp, const float *__restrict__ rp)
 {
 #pragma unroll
     for (int u = 0; u < 8; u += 2) {
-        const float4 rr = *reinterpret_cast<const float4 *>(rp + u);
-        const float2 r0 = make_float2(rr.x, rr.y), r1 = make_float2(rr.z, rr.w);
+        const float2 rr = *reinterpret_cast<const float2 *>(rp + u);              // r_w of the two widths: scalar-broadcast operands of FMUL2
+        const float2 r0 = make_float2(rr.x, rr.x), r1 = make_float2(rr.y, rr.y);
         const float2 n0 = zp[u], n1 = zp[u + 1];
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) {
@@ -172,8 +172,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
     float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
     float2 *P2  = reinterpret_cast<float2 *>(smem_raw + lay.p2);      // prefix sums of y: (sub-tile A, sub-tile B), zpad layout
     float2 *scan = reinterpret_cast<float2 *>(smem_raw + lay.scan);   // [2][4] per-warp totals of the tile prefix scan
-    float2 *rt2 = reinterpret_cast<float2 *>(smem_raw + lay.rt2);     // (r_w, r_w): operand of FMUL2
-    float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);      // r_w plain: LDS.128 in the width search
+    float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);      // r_w = 1 / sigma_w
 
     const int tid = threadIdx.x;
     const int lane = tid & 31, wid = tid >> 5;
@@ -187,7 +186,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
     const float2 mu_hi2 = make_float2(-mu_hi, -mu_hi), mu_lo2 = make_float2(-mu_lo, -mu_lo);
     const float NINF = __int_as_float(0xff800000);
 
-    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) { float r = __ldg(table + w); rt2[w] = make_float2(r, r); rtf[w] = r; }
+    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
 
     auto prefetch = [&](int64_t tile) { stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile, LRAW, tid); };
 
@@ -272,7 +271,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
         // ---- main loop: blocks of 8 widths, the running maximum ping-pongs between bestA and bestB ---------------------
         {
             const float2 *zp = Z + 9 * (tid + 1);                // zpad(8 tid + 8 kb + 8 + u) = 9 (tid + kb + 1) + u
-            const float2 *rp = rt2;
+            const float *rp = rtf;
             int kb = 0;
             for (; kb + 2 <= nblk; kb += 2) {
                 sweep8(B, W, bestA, bestB, zp, rp);
@@ -365,14 +364,13 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
 // in the order of the main loop (same fp32 adds and multiplies, so the values are bit-identical) and takes the first
 // width whose SNR equals the maximum: the smallest arg-max (A7).
 struct FusedSmem {
-    int z, raw, rt2, rtf, total;
+    int z, raw, rtf, total;
     __host__ __device__ explicit FusedSmem(int nmax)
     {
         const int H = sw_halo(nmax), R = sw_rt_len(nmax);
         z = 0;
         raw = z + round_up((zpad(SW_SUB + H) + 1) * 8, 16);
-        rt2 = raw + round_up((SW_TILE + H) * 4, 16);
-        rtf = rt2 + R * 8;
+        rtf = raw + round_up((SW_TILE + H) * 4, 16);
         total = rtf + round_up(R * 4, 16);
     }
 };
@@ -397,7 +395,6 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
     const FusedSmem lay(nmax);
     float2 *Z   = reinterpret_cast<float2 *>(smem_raw + lay.z);
     float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
-    float2 *rt2 = reinterpret_cast<float2 *>(smem_raw + lay.rt2);
     float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);
 
     const int tid = threadIdx.x;
@@ -410,7 +407,7 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
     const float2 mu_hi2 = make_float2(-mu_hi, -mu_hi), mu_lo2 = make_float2(-mu_lo, -mu_lo);
     const float NINF = __int_as_float(0xff800000);
 
-    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) { float r = __ldg(table + w); rt2[w] = make_float2(r, r); rtf[w] = r; }
+    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
 
     int64_t tile = blockIdx.x;
     if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile, LRAW, tid);
@@ -444,7 +441,7 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
         for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); }
         {
             const float2 *zp = Z + 9 * (tid + 1);
-            const float2 *rp = rt2;
+            const float *rp = rtf;
             for (int kb = 0; kb < nblk; ++kb, zp += 9, rp += 8) sweep8(B, W, best, best, zp, rp);
         }
 
