@@ -113,9 +113,10 @@ stats_partial(const float *__restrict__ x, int64_t n_rows, int64_t n_t, int64_t 
 }
 
 // ---- sigma_Nmax: population std of the Nmax-sample boxcar SUMS over every full window (reading A11) ----
-// One tile = 4096 consecutive windows of one row (+ nmax-1 halo samples) staged in shared memory.  Each thread owns
-// 16 consecutive windows: the first sum is taken directly (fp64), the next 15 slide (+x[t+nmax] - x[t], fp64), the
-// sums go through eq. 1 (fp64) and the warp's runs are merged with eq. 2.
+// One tile = 4096 consecutive windows of one row (+ nmax-1 halo samples) staged in shared memory, together with its
+// tile-local fp64 prefix sums P (block scan).  Each thread owns 16 consecutive windows: the first sum is
+// P[t+nmax] - P[t], the next 15 slide (+x[t+nmax] - x[t], fp64), the sums go through eq. 1 (fp64) and the warp's runs
+// are merged with eq. 2.
 constexpr int SB_WIN = 16;
 constexpr int SB_TILE = ST_THREADS * SB_WIN;
 __host__ __device__ __forceinline__ int sb_pad(int i) { return i + (i >> 4); }   // lane stride 17 words: conflict-free
@@ -124,13 +125,17 @@ __global__ void __launch_bounds__(ST_THREADS)
 stats_boxcar_partial(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax,
                      Tri *__restrict__ partials)
 {
-    extern __shared__ float xs[];
+    extern __shared__ __align__(16) unsigned char sb_smem[];
     __shared__ Tri warp_acc[ST_THREADS / 32];
+    __shared__ double wtot[ST_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    double *Pd = reinterpret_cast<double *>(sb_smem);                              // [span + 1] prefix sums
+    float *xs = reinterpret_cast<float *>(Pd + (SB_TILE + nmax));                  // [sb_pad(span) + 1] samples
     const int64_t nwin = n_t - nmax + 1;
     const int64_t tpr = (nwin + SB_TILE - 1) / SB_TILE;
     const int64_t total = n_dm * tpr;
     const int span = SB_TILE + nmax - 1;
+    const int seg = (span + ST_THREADS - 1) / ST_THREADS;
     Tri acc = {0.0, 0.0, 0.0};
 
     for (int64_t c = blockIdx.x; c < total; c += gridDim.x) {
@@ -139,11 +144,25 @@ stats_boxcar_partial(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int
         __syncthreads();
         for (int i = tid; i < span; i += ST_THREADS) xs[sb_pad(i)] = (t0 + i < n_t) ? __ldg(rp + t0 + i) : 0.0f;
         __syncthreads();
+        {   // P[i] = xs[0] + ... + xs[i-1] in fp64: per-thread segment sums, warp scan, cross-warp offsets
+            const int lo = min(tid * seg, span), hi = min(lo + seg, span);
+            double run = 0.0;
+            for (int i = lo; i < hi; ++i) run += (double)xs[sb_pad(i)];
+            double inc = run;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { const double o = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += o; }
+            if (lane == 31) wtot[wid] = inc;
+            __syncthreads();
+            double off = inc - run;
+            for (int w = 0; w < wid; ++w) off += wtot[w];
+            for (int i = lo; i < hi; ++i) { Pd[i] = off; off += (double)xs[sb_pad(i)]; }
+            if (hi == span && lo < hi) Pd[span] = off;           // the one thread whose non-empty segment ends the tile
+        }
+        __syncthreads();
         const int w0 = tid * SB_WIN;
         Tri t = {0.0, 0.0, 0.0};
         if (t0 + w0 < nwin) {
-            double B = 0.0;
-            for (int k = 0; k < nmax; ++k) B += (double)xs[sb_pad(w0 + k)];
+            double B = Pd[w0 + nmax] - Pd[w0];
             t.m = 1.0; t.T = B; t.S = 0.0;
 #pragma unroll
             for (int r = 1; r < SB_WIN; ++r) {
@@ -246,7 +265,7 @@ cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
         int64_t nwin = n_t - nmax_for_sigma + 1;
         int64_t tiles = n_dm * ((nwin + SB_TILE - 1) / SB_TILE);
         gb = (int)(tiles < ST_GRID ? tiles : ST_GRID);
-        size_t smem = (size_t)(sb_pad(SB_TILE + nmax_for_sigma) + 1) * sizeof(float);
+        size_t smem = (size_t)(SB_TILE + nmax_for_sigma) * sizeof(double) + (size_t)(sb_pad(SB_TILE + nmax_for_sigma) + 1) * sizeof(float);
         cudaError_t e = cudaFuncSetAttribute(stats_boxcar_partial, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         stats_boxcar_partial<<<gb, ST_THREADS, smem, s>>>(x, n_dm, n_t, row_stride, nmax_for_sigma, pb);
