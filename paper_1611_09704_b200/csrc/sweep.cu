@@ -38,6 +38,7 @@ constexpr int SW_THREADS = 128;
 constexpr int SW_R       = 8;                        // samples per thread per sub-tile
 constexpr int SW_SUB     = SW_THREADS * SW_R;        // 1024
 constexpr int SW_TILE    = 2 * SW_SUB;               // 2048 samples per tile
+constexpr int SW_NARROW_NMAX = 24;                   // nmax up to here takes the tagged-maximum kernel (measured crossover on B200: 24..28)
 
 __host__ __device__ inline int zpad(int i) { return i + (i >> 3); }          // one pad float2 per 8: lane stride 72 B
 __host__ __device__ inline int sw_nblk(int nmax) { return (nmax + 7) >> 3; }  // blocks of 8 widths
@@ -158,6 +159,45 @@ __device__ __forceinline__ void note_block(const float2 (&now)[SW_R], const floa
     for (int j = 0; j < SW_R; ++j) {
         w0x[j] = (now[j].x > old[j].x) ? w0 : w0x[j];
         w0y[j] = (now[j].y > old[j].y) ? w0 : w0y[j];
+    }
+}
+
+// SNR (f32) and width (u16) of a thread's 8 + 8 samples: 16-byte streaming stores where the row is aligned and whole
+__device__ __forceinline__ void store_planes(float *__restrict__ snr, uint16_t *__restrict__ width, int64_t row, int64_t row_stride,
+                                             int64_t n_t, int64_t ta, const float2 (&best)[SW_R], const int (&wx)[SW_R], const int (&wy)[SW_R])
+{
+    const int64_t tb = ta + SW_SUB;
+    float *oa = snr + row * row_stride + ta, *ob = snr + row * row_stride + tb;
+    const bool v4 = ((reinterpret_cast<uintptr_t>(snr + row * row_stride) & 15) == 0);
+    if (v4 && ta + 7 < n_t) {
+        __stcs(reinterpret_cast<float4 *>(oa), make_float4(best[0].x, best[1].x, best[2].x, best[3].x));
+        __stcs(reinterpret_cast<float4 *>(oa) + 1, make_float4(best[4].x, best[5].x, best[6].x, best[7].x));
+    } else {
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) oa[j] = best[j].x;
+    }
+    if (v4 && tb + 7 < n_t) {
+        __stcs(reinterpret_cast<float4 *>(ob), make_float4(best[0].y, best[1].y, best[2].y, best[3].y));
+        __stcs(reinterpret_cast<float4 *>(ob) + 1, make_float4(best[4].y, best[5].y, best[6].y, best[7].y));
+    } else {
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) ob[j] = best[j].y;
+    }
+    if (width) {
+        uint16_t *wa = width + row * row_stride + ta, *wb = width + row * row_stride + tb;
+        const bool w8 = ((reinterpret_cast<uintptr_t>(width + row * row_stride) & 15) == 0);
+        if (w8 && ta + 7 < n_t)
+            __stcs(reinterpret_cast<uint4 *>(wa), make_uint4(wx[0] | (wx[1] << 16), wx[2] | (wx[3] << 16), wx[4] | (wx[5] << 16), wx[6] | (wx[7] << 16)));
+        else {
+#pragma unroll
+            for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) wa[j] = (uint16_t)wx[j];
+        }
+        if (w8 && tb + 7 < n_t)
+            __stcs(reinterpret_cast<uint4 *>(wb), make_uint4(wy[0] | (wy[1] << 16), wy[2] | (wy[3] << 16), wy[4] | (wy[5] << 16), wy[6] | (wy[7] << 16)));
+        else {
+#pragma unroll
+            for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) wb[j] = (uint16_t)wy[j];
+        }
     }
 }
 
@@ -319,40 +359,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
             for (int j = 0; j < SW_R; ++j) best[j] = make_float2(rtf[0], rtf[0]);
         }
 
-        // ---- results ----------------------------------------------------------------------------------------------
-        const int64_t ta = T0 + SW_R * tid, tb = ta + SW_SUB;
-        float *oa = snr + row * row_stride + ta, *ob = snr + row * row_stride + tb;
-        const bool v4 = ((reinterpret_cast<uintptr_t>(snr + row * row_stride) & 15) == 0);
-        if (v4 && ta + 7 < n_t) {
-            __stcs(reinterpret_cast<float4 *>(oa), make_float4(best[0].x, best[1].x, best[2].x, best[3].x));
-            __stcs(reinterpret_cast<float4 *>(oa) + 1, make_float4(best[4].x, best[5].x, best[6].x, best[7].x));
-        } else {
-#pragma unroll
-            for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) oa[j] = best[j].x;
-        }
-        if (v4 && tb + 7 < n_t) {
-            __stcs(reinterpret_cast<float4 *>(ob), make_float4(best[0].y, best[1].y, best[2].y, best[3].y));
-            __stcs(reinterpret_cast<float4 *>(ob) + 1, make_float4(best[4].y, best[5].y, best[6].y, best[7].y));
-        } else {
-#pragma unroll
-            for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) ob[j] = best[j].y;
-        }
-        if (width) {
-            uint16_t *wa = width + row * row_stride + ta, *wb = width + row * row_stride + tb;
-            const bool w8 = ((reinterpret_cast<uintptr_t>(width + row * row_stride) & 15) == 0);
-            if (w8 && ta + 7 < n_t)
-                __stcs(reinterpret_cast<uint4 *>(wa), make_uint4(wx[0] | (wx[1] << 16), wx[2] | (wx[3] << 16), wx[4] | (wx[5] << 16), wx[6] | (wx[7] << 16)));
-            else {
-#pragma unroll
-                for (int j = 0; j < SW_R; ++j) if (ta + j < n_t) wa[j] = (uint16_t)wx[j];
-            }
-            if (w8 && tb + 7 < n_t)
-                __stcs(reinterpret_cast<uint4 *>(wb), make_uint4(wy[0] | (wy[1] << 16), wy[2] | (wy[3] << 16), wy[4] | (wy[5] << 16), wy[6] | (wy[7] << 16)));
-            else {
-#pragma unroll
-                for (int j = 0; j < SW_R; ++j) if (tb + j < n_t) wb[j] = (uint16_t)wy[j];
-            }
-        }
+        store_planes(snr, width, row, row_stride, n_t, T0 + SW_R * tid, best, wx, wy);
     }
     cp_async_commit_wait_all();
 }
@@ -468,6 +475,111 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
     cp_async_commit_wait_all();
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Narrow searches (nmax <= SW_NARROW_NMAX; the tag has room for 32 widths): the fixed per-sample cost of the general kernel (prefix scan + width search, about 100
+// clocks per 32 samples) is larger than the width loop itself, so here the arg-max rides along with the maximum:
+// beside the exact running maximum a second one is kept over TAGGED values, (bits(s) & ~31) | (32 - w).  A larger
+// tag is a smaller width, so exact ties keep the smallest width (A7); values closer than 32 ulp (4e-6 relative, far
+// inside the 1e-3 tie tolerance of DESIGN.md section 5) may resolve either way.  The SNR written is the exact maximum.
+// A tagged -inf (a window past the row end) is a NaN, which FMNMX drops.  No scan, no width search, no bookkeeping.
+template <int KB>
+__device__ __forceinline__ void sweep8_tagged(float2 (&B)[SW_R], float2 (&W)[SW_R], float2 (&best)[SW_R], float2 (&tbest)[SW_R],
+                                              const float2 *__restrict__ zp, const float *__restrict__ rp)
+{
+#pragma unroll
+    for (int u = 0; u < 8; u += 2) {
+        const float2 rr = *reinterpret_cast<const float2 *>(rp + u);
+        const float2 r0 = make_float2(rr.x, rr.x), r1 = make_float2(rr.y, rr.y);
+        const float2 n0 = zp[u], n1 = zp[u + 1];
+        constexpr int MASK = ~31;
+        const int c0 = 32 - (8 * KB + u + 1), c1 = c0 - 1;              // 32 - w for the two widths of this step
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) {
+            B[j] = __fadd2_rn(B[j], W[(j + u) & 7]);
+            const float2 s0 = __fmul2_rn(B[j], r0);
+            B[j] = __fadd2_rn(B[j], (j == SW_R - 1) ? n0 : W[(j + u + 1) & 7]);
+            const float2 s1 = __fmul2_rn(B[j], r1);
+            best[j].x = fmax3(best[j].x, s0.x, s1.x);
+            best[j].y = fmax3(best[j].y, s0.y, s1.y);
+            tbest[j].x = fmax3(tbest[j].x, __int_as_float((__float_as_int(s0.x) & MASK) | c0), __int_as_float((__float_as_int(s1.x) & MASK) | c1));
+            tbest[j].y = fmax3(tbest[j].y, __int_as_float((__float_as_int(s0.y) & MASK) | c0), __int_as_float((__float_as_int(s1.y) & MASK) | c1));
+        }
+        W[u] = n0;
+        W[u + 1] = n1;
+    }
+}
+
+__global__ void __launch_bounds__(SW_THREADS, 5)
+boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
+                        const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
+                        float *__restrict__ snr, uint16_t *__restrict__ width)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const FusedSmem lay(nmax);
+    float2 *Z   = reinterpret_cast<float2 *>(smem_raw + lay.z);
+    float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
+    float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);
+
+    const int tid = threadIdx.x;
+    const int nblk = sw_nblk(nmax);
+    const int H = sw_halo(nmax);
+    const int LRAW = SW_TILE + H, LZ = SW_SUB + H;
+    const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
+    const double mu = st->mean;
+    const float mu_hi = (float)mu, mu_lo = (float)(mu - (double)mu_hi);
+    const float2 mu_hi2 = make_float2(-mu_hi, -mu_hi), mu_lo2 = make_float2(-mu_lo, -mu_lo);
+    const float NINF = __int_as_float(0xff800000);
+
+    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
+
+    int64_t tile = blockIdx.x;
+    if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile, LRAW, tid);
+
+    for (; tile < total_tiles; tile += gridDim.x) {
+        const int64_t row = tile / tiles_per_row;
+        const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
+        cp_async_commit_wait_all();
+        __syncthreads();                           // raw tile landed; everyone is done with the previous Z
+
+        float2 B[SW_R], W[SW_R], best[SW_R], tbest[SW_R];
+        for (int part = 0; part < nparts; ++part) {
+            const int g = part * SW_THREADS + tid;
+            if (8 * g < LZ) {
+                const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
+                const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
+                float2 v[SW_R] = {make_float2(a0.x, b0.x), make_float2(a0.y, b0.y), make_float2(a0.z, b0.z), make_float2(a0.w, b0.w),
+                                  make_float2(a1.x, b1.x), make_float2(a1.y, b1.y), make_float2(a1.z, b1.z), make_float2(a1.w, b1.w)};
+#pragma unroll
+                for (int j = 0; j < SW_R; ++j) {
+                    v[j] = __fadd2_rn(__fadd2_rn(v[j], mu_hi2), mu_lo2);
+                    Z[9 * g + j] = v[j];
+                    if (part == 0) W[j] = v[j];
+                }
+            }
+        }
+        __syncthreads();                           // Z complete; raw is free again
+        if (tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile + gridDim.x, LRAW, tid);
+
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); tbest[j] = make_float2(NINF, NINF); }
+        const float2 *zp = Z + 9 * (tid + 1);
+        sweep8_tagged<0>(B, W, best, tbest, zp, rtf);
+        if (nblk > 1) sweep8_tagged<1>(B, W, best, tbest, zp + 9, rtf + 8);
+        if (nblk > 2) sweep8_tagged<2>(B, W, best, tbest, zp + 18, rtf + 16);
+        if (nblk > 3) sweep8_tagged<3>(B, W, best, tbest, zp + 27, rtf + 24);
+
+        int wx[SW_R], wy[SW_R];
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) { wx[j] = 32 - (__float_as_int(tbest[j].x) & 31); wy[j] = 32 - (__float_as_int(tbest[j].y) & 31); }
+        if (rtf[0] != rtf[0]) {                     // NaN table (LINEAR mode fed stats of another Nmax) must surface
+#pragma unroll
+            for (int j = 0; j < SW_R; ++j) { best[j] = make_float2(rtf[0], rtf[0]); wx[j] = 1; wy[j] = 1; }
+        }
+        store_planes(snr, width, row, row_stride, n_t, T0 + SW_R * tid, best, wx, wy);
+    }
+    cp_async_commit_wait_all();
+}
+
 template <typename K>
 static cudaError_t persistent_grid(K kernel, int smem, int64_t tiles, unsigned *grid)
 {
@@ -497,6 +609,10 @@ cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
         if ((e = persistent_grid(boxcar_search_fused, lay.total, tiles, &grid)) != cudaSuccess) return e;
         boxcar_search_fused<<<grid, SW_THREADS, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax,
                                                                 threshold, out, capacity, d_count);
+    } else if (nmax <= SW_NARROW_NMAX) {
+        const FusedSmem lay(nmax);
+        if ((e = persistent_grid(boxcar_snr_sweep_narrow, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep_narrow<<<grid, SW_THREADS, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
     } else {
         const SweepSmem lay(nmax);
         if ((e = persistent_grid(boxcar_snr_sweep, lay.total, tiles, &grid)) != cudaSuccess) return e;

@@ -123,6 +123,7 @@ def test_sweep_integer_data_forced_stats(P, n_dm, n_t, nmax):
 @pytest.mark.parametrize("n_dm,n_t,nmax,mu,sigma", [
     (4, 4096, 32, 0.0, 1.0), (3, 6000, 128, 0.0, 1.0), (3, 5000, 64, 100.0, 20.0), (2, 7777, 512, 0.0, 1.0),
     (2, 4100, 100, -1000.0, 1.0), (64, 2048, 8, 0.0, 1.0),
+    (3, 5000, 16, 100.0, 20.0), (2, 3001, 24, 0.0, 1.0), (2, 4099, 25, 0.0, 1.0),      # both sides of the narrow-kernel switch
 ])
 def test_sweep_noise(P, n_dm, n_t, nmax, mu, sigma):
     x = (mu + sigma * rng(300 + nmax).standard_normal((n_dm, n_t))).astype(np.float32)
