@@ -84,6 +84,8 @@ spd_status spd_stats_merge(const spd_stats_t *d_parts, int count, spd_stats_t *d
  *   d_snr[d][t] = max_N SNR_N(t),  d_width[d][t] = the smallest N attaining it.
  * mu, sigma (and sigma_nmax for the LINEAR modes) are read from *d_stats on the device; a LINEAR mode
  * fed stats whose nmax_of_sigma != nmax yields an all-NaN SNR plane (it cannot be caught without a sync).
+ * Widths whose fp32 SNRs differ by less than about 4e-6 relative (rounding of the running sums) count as tied and
+ * either may be reported; an exact tie reports the smallest.  d_snr is always the maximum itself.
  * Requires 1 <= nmax <= min(n_t, 4096) (shared-memory bound of the tile).  d_width may be NULL (plane not written). */
 spd_status spd_boxcar_snr(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
                           const spd_stats_t *d_stats, int nmax, spd_sigma_mode mode,
