@@ -99,13 +99,27 @@ cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, f
     return cudaGetLastError();
 }
 
+// Position of a tile in the persistent walk: (row, tile-in-row), advanced by the grid size without 64-bit divisions
+struct TilePos {
+    int64_t row; int tr;
+    __device__ __forceinline__ TilePos(unsigned first, int tiles_per_row) : row(first / (unsigned)tiles_per_row), tr((int)(first % (unsigned)tiles_per_row)) {}
+    __device__ __forceinline__ TilePos next(unsigned step, int tiles_per_row) const
+    {
+        TilePos p = *this;
+        unsigned t = (unsigned)p.tr + step;
+        if (t >= (unsigned)tiles_per_row) { const unsigned q = t / (unsigned)tiles_per_row; p.row += q; t -= q * (unsigned)tiles_per_row; }
+        p.tr = (int)t;
+        return p;
+    }
+};
+
 // raw tile -> shared memory, asynchronously where the 16-byte fast path applies; past the row end -> -inf
 __device__ __forceinline__ void stage_tile(float *__restrict__ raw, const float *__restrict__ x, int64_t n_t, int64_t row_stride,
-                                           int tiles_per_row, int64_t tile, int LRAW, int tid)
+                                           const TilePos &pos_, int LRAW, int tid)
 {
     const float NINF = __int_as_float(0xff800000);
-    const int64_t row = tile / tiles_per_row;
-    const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
+    const int64_t row = pos_.row;
+    const int64_t T0 = (int64_t)pos_.tr * SW_TILE;
     const float *rowp = x + row * row_stride;
     const bool vec = ((reinterpret_cast<uintptr_t>(rowp) & 15) == 0);
     if (vec && T0 + LRAW <= n_t) {                       // interior tile: no bounds checks
@@ -228,14 +242,14 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
 
     for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
 
-    auto prefetch = [&](int64_t tile) { stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile, LRAW, tid); };
-
     int64_t tile = blockIdx.x;
-    if (tile < total_tiles) prefetch(tile);
+    TilePos pos(blockIdx.x, tiles_per_row);
+    if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);
 
     for (; tile < total_tiles; tile += gridDim.x) {
-        const int64_t row = tile / tiles_per_row;
-        const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
+        const int64_t row = pos.row;
+        const int64_t T0 = (int64_t)pos.tr * SW_TILE;
+        pos = pos.next(gridDim.x, tiles_per_row);                                  // the tile after this one
         cp_async_commit_wait_all();
         __syncthreads();                           // raw tile landed; everyone is done with the previous Z / P
 
@@ -291,7 +305,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
                 off.x = __shfl_up_sync(0xffffffffu, inc.x, 1); off.y = __shfl_up_sync(0xffffffffu, inc.y, 1);
                 if (lane == 0) off = make_float2(0.f, 0.f);
                 __syncthreads();                                 // totals visible; this part of raw is consumed, of Z written
-                if (part == nparts - 1 && tile + gridDim.x < total_tiles) prefetch(tile + gridDim.x);   // raw is free again
+                if (part == nparts - 1 && tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);   // raw is free again
                 off = __fadd2_rn(off, carry);
 #pragma unroll
                 for (int w = 0; w < SW_THREADS / 32; ++w) {
@@ -345,10 +359,12 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
                 float s[8];
 #pragma unroll
                 for (int g = 0; g < 8; ++g) { const int c = j + g + 1; s[g] = (pe[2 * (c + (c >> 3))] - p0h) * r[g]; }
-                const float m = fmaxf(fmax3(fmax3(s[0], s[1], s[2]), s[3], s[4]), fmax3(s[5], s[6], s[7]));
-                int w = 0;
+                // the position inside the block rides in the 3 low mantissa bits (7 - g: ties keep the smallest width);
+                // a tagged -inf or NaN (width past the row end / past nmax) is a NaN, which FMNMX drops
 #pragma unroll
-                for (int g = 7; g >= 0; --g) w = (s[g] == m) ? g : w;
+                for (int g = 0; g < 8; ++g) s[g] = __int_as_float((__float_as_int(s[g]) & ~7) | (7 - g));
+                const float m = fmaxf(fmax3(fmax3(s[0], s[1], s[2]), s[3], s[4]), fmax3(s[5], s[6], s[7]));
+                const int w = 7 - (__float_as_int(m) & 7);
                 if (h) wy[j] = w0 + w + 1; else wx[j] = w0 + w + 1;
             }
         }
@@ -392,7 +408,7 @@ __device__ __noinline__ int replay_width(const float *__restrict__ zh, int pos, 
     return nmax;                                   // not reached for finite input
 }
 
-__global__ void __launch_bounds__(SW_THREADS, 5)
+__global__ void __launch_bounds__(SW_THREADS, 4)
 boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                     const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
                     float threshold, spd_candidate_t *__restrict__ cand, unsigned long long capacity,
@@ -417,11 +433,13 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
     for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
 
     int64_t tile = blockIdx.x;
-    if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile, LRAW, tid);
+    TilePos pos(blockIdx.x, tiles_per_row);
+    if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);
 
     for (; tile < total_tiles; tile += gridDim.x) {
-        const int64_t row = tile / tiles_per_row;
-        const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
+        const int64_t row = pos.row;
+        const int64_t T0 = (int64_t)pos.tr * SW_TILE;
+        pos = pos.next(gridDim.x, tiles_per_row);                                  // the tile after this one
         cp_async_commit_wait_all();
         __syncthreads();                           // raw tile landed; everyone is done with the previous Z
 
@@ -442,7 +460,7 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
             }
         }
         __syncthreads();                           // Z complete; raw is free again
-        if (tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile + gridDim.x, LRAW, tid);
+        if (tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);
 
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); }
@@ -533,11 +551,13 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
     for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
 
     int64_t tile = blockIdx.x;
-    if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile, LRAW, tid);
+    TilePos pos(blockIdx.x, tiles_per_row);
+    if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);
 
     for (; tile < total_tiles; tile += gridDim.x) {
-        const int64_t row = tile / tiles_per_row;
-        const int64_t T0 = (tile - row * tiles_per_row) * SW_TILE;
+        const int64_t row = pos.row;
+        const int64_t T0 = (int64_t)pos.tr * SW_TILE;
+        pos = pos.next(gridDim.x, tiles_per_row);                                  // the tile after this one
         cp_async_commit_wait_all();
         __syncthreads();                           // raw tile landed; everyone is done with the previous Z
 
@@ -558,7 +578,7 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
             }
         }
         __syncthreads();                           // Z complete; raw is free again
-        if (tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, tiles_per_row, tile + gridDim.x, LRAW, tid);
+        if (tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);
 
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); tbest[j] = make_float2(NINF, NINF); }
