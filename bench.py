@@ -180,15 +180,10 @@ def run_ours(args):
     h_x = torch.empty((n_dm, n_t), dtype=torch.float32, pin_memory=True)
     gen.make_array(cfg, out=h_x.numpy(), threads=max(1, (os.cpu_count() or 1) // max(1, world)), row_hi=n_dm)
     t_gen = time.time() - t_gen
-    arena = torch.empty(P.search_host_arena_bytes(n_dm, n_t, nmax, cap), dtype=torch.uint8, device=dev)
-    # device-resident leg uses the arena's own regions (same layout as spd_search_host): x | snr | width
-    def region(off, nbytes, dtype, shape):
-        return arena[off:off + nbytes].view(dtype).view(shape)
-    a256 = lambda v: (v + 255) // 256 * 256
-    o_x, o_snr, o_w = 0, a256(n * 4), a256(n * 4) * 2
-    d_x = region(o_x, n * 4, torch.float32, (n_dm, n_t))
-    d_snr = region(o_snr, n * 4, torch.float32, (n_dm, n_t))
-    d_w = region(o_w, n * 2, torch.uint16, (n_dm, n_t))
+    arena = torch.empty(P.search_host_arena_bytes(n_dm, n_t, nmax, cap), dtype=torch.uint8, device=dev)   # of the e2e leg
+    d_x = torch.empty((n_dm, n_t), dtype=torch.float32, device=dev)
+    d_snr = torch.empty((n_dm, n_t), dtype=torch.float32, device=dev)
+    d_w = torch.empty((n_dm, n_t), dtype=torch.uint16, device=dev)
     d_x.copy_(h_x, non_blocking=True)
     st = P.new_stats(dev)
     ws = P.new_workspace(n_dm, n_t, nmax, dev)
@@ -318,7 +313,7 @@ def run_ours(args):
             "clocks": clocks,
             "e2e": {"value": world * n / (ms_e2e * 1e-3), "unit": "samples/s", "ms_per_step": ms_e2e, "steps": e2e_steps,
                     "h2d_bytes_per_step": n * 4, "d2h_bytes_per_step": 8 + P.STATS_DTYPE.itemsize + 16 * min(hits_e2e, cap),
-                    "api": "spd_search_host (pinned host buffers)"},
+                    "api": "spd_search_host (pinned host buffers; H2D, spd_stats, spd_search_fused, D2H of statistics, count and records)"},
             "gpu_launches": launches_per_step * args.steps,
             "roofline": roof,
             "cpu_baseline": cpu,

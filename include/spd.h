@@ -111,11 +111,11 @@ spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t
 /* Device bytes spd_search_host needs in d_arena for this shape and capacity. */
 size_t spd_search_host_arena_bytes(int64_t n_dm, int64_t n_t, int nmax, uint64_t capacity);
 
-/* The whole path from HOST buffers: copies h_x (row_stride = n_t) to the device, runs spd_stats,
- * spd_boxcar_snr and spd_candidates, and copies the statistics, the hit count and the first
- * min(count, capacity) records back.  h_x / h_out / h_count / h_stats are HOST pointers (pinned memory
- * makes the copies asynchronous); d_arena is a caller-owned DEVICE buffer of >=
- * spd_search_host_arena_bytes().  This call SYNCHRONISES `stream` before it returns. */
+/* The whole path from HOST buffers: copies h_x (row_stride = n_t) to the device, runs spd_stats and
+ * spd_search_fused (the list is the product; the planes are not materialised), and copies the
+ * statistics, the hit count and the first min(count, capacity) records back.  h_x / h_out / h_count /
+ * h_stats are HOST pointers (pinned memory makes the copies asynchronous); d_arena is a caller-owned DEVICE
+ * buffer of >= spd_search_host_arena_bytes(), 256-byte aligned.  This call SYNCHRONISES `stream` before it returns. */
 spd_status spd_search_host(const float *h_x, int64_t n_dm, int64_t n_t, int nmax, spd_sigma_mode mode,
                            float threshold, spd_candidate_t *h_out, uint64_t capacity,
                            unsigned long long *h_count, spd_stats_t *h_stats,

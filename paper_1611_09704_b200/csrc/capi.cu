@@ -104,13 +104,13 @@ spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t
     return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
 }
 
-// arena layout of spd_search_host: x | snr | width | candidates | stats | count | workspace
+// arena layout of spd_search_host: x | candidates | stats | count | workspace
 size_t spd_search_host_arena_bytes(int64_t n_dm, int64_t n_t, int nmax, uint64_t capacity)
 {
     if (n_dm < 1 || n_t < 1 || nmax < 1 || nmax > NMAX_API_LIMIT) return 0;
     const size_t n = (size_t)n_dm * (size_t)n_t;
-    return align_up(n * 4, 256) + align_up(n * 4, 256) + align_up(n * 2, 256) +
-           align_up((size_t)capacity * sizeof(spd_candidate_t), 256) + 256 + 256 + spd_workspace_bytes(n_dm, n_t, nmax);
+    return align_up(n * 4, 256) + align_up((size_t)capacity * sizeof(spd_candidate_t), 256) + 256 + 256 +
+           spd_workspace_bytes(n_dm, n_t, nmax);
 }
 
 spd_status spd_search_host(const float *h_x, int64_t n_dm, int64_t n_t, int nmax, spd_sigma_mode mode,
@@ -126,8 +126,6 @@ spd_status spd_search_host(const float *h_x, int64_t n_dm, int64_t n_t, int nmax
     const size_t n = (size_t)n_dm * (size_t)n_t;
     unsigned char *p = reinterpret_cast<unsigned char *>(d_arena);
     float *d_x = reinterpret_cast<float *>(p);                 p += align_up(n * 4, 256);
-    float *d_snr = reinterpret_cast<float *>(p);               p += align_up(n * 4, 256);
-    uint16_t *d_width = reinterpret_cast<uint16_t *>(p);       p += align_up(n * 2, 256);
     spd_candidate_t *d_out = reinterpret_cast<spd_candidate_t *>(p); p += align_up((size_t)capacity * sizeof(spd_candidate_t), 256);
     spd_stats_t *d_stats = reinterpret_cast<spd_stats_t *>(p); p += 256;
     unsigned long long *d_count = reinterpret_cast<unsigned long long *>(p); p += 256;
@@ -137,9 +135,7 @@ spd_status spd_search_host(const float *h_x, int64_t n_dm, int64_t n_t, int nmax
     if (cudaMemcpyAsync(d_x, h_x, n * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPD_ERR_CUDA;
     spd_status st = spd_stats(d_x, n_dm, n_t, n_t, mode == SPD_SIGMA_SQRT ? 0 : nmax, d_stats, d_ws, ws_bytes, stream);
     if (st != SPD_OK) return st;
-    st = spd_boxcar_snr(d_x, n_dm, n_t, n_t, d_stats, nmax, mode, d_snr, d_width, d_ws, ws_bytes, stream);
-    if (st != SPD_OK) return st;
-    st = spd_candidates(d_snr, d_width, n_dm, n_t, n_t, threshold, d_out, capacity, d_count, stream);
+    st = spd_search_fused(d_x, n_dm, n_t, n_t, d_stats, nmax, mode, threshold, d_out, capacity, d_count, d_ws, ws_bytes, stream);
     if (st != SPD_OK) return st;
     if (h_stats && cudaMemcpyAsync(h_stats, d_stats, sizeof(spd_stats_t), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
     if (cudaMemcpyAsync(h_count, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;

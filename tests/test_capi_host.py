@@ -47,7 +47,7 @@ def test_workspace_sizes(L):
     assert L.spd_workspace_bytes(64, 16384, 32) >= 2 * 2048 * 24
     assert L.spd_workspace_bytes(0, 16384, 32) == 0 and L.spd_workspace_bytes(1, 1, 5000) == 0
     n = 6000 * 262144
-    assert L.spd_search_host_arena_bytes(6000, 262144, 128, 1 << 20) >= n * 10 + (16 << 20)
+    assert L.spd_search_host_arena_bytes(6000, 262144, 128, 1 << 20) >= n * 4 + (16 << 20)      # x + records (+ stats, count, workspace)
 
 
 def test_argument_validation_needs_no_device(L):
