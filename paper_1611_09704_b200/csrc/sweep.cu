@@ -272,38 +272,42 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
             for (int part = 0; part < nparts; ++part) {
                 const int g = part * SW_THREADS + tid;           // group of 8 positions: 8 g .. 8 g + 7
                 const bool act = 8 * g < LZ;
+                const bool wact = 8 * (g - lane) < LZ;           // warp-uniform: any lane of this warp active (the halo part keeps one warp busy)
                 float2 v[SW_R];
-                if (act) {
-                    const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
-                    const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
-                    v[0] = make_float2(a0.x, b0.x); v[1] = make_float2(a0.y, b0.y); v[2] = make_float2(a0.z, b0.z); v[3] = make_float2(a0.w, b0.w);
-                    v[4] = make_float2(a1.x, b1.x); v[5] = make_float2(a1.y, b1.y); v[6] = make_float2(a1.z, b1.z); v[7] = make_float2(a1.w, b1.w);
-#pragma unroll
-                    for (int j = 0; j < SW_R; ++j) {
-                        v[j] = __fadd2_rn(__fadd2_rn(v[j], mu_hi2), mu_lo2);
-                        Z[9 * g + j] = v[j];                     // zpad(8 g + j) = 9 g + j
-                    }
-                } else {
-#pragma unroll
-                    for (int j = 0; j < SW_R; ++j) v[j] = make_float2(0.f, 0.f);
-                }
-                if (part == 0) {
-#pragma unroll
-                    for (int j = 0; j < SW_R; ++j) W[j] = v[j];
-                }
-#pragma unroll
-                for (int j = 1; j < SW_R; ++j) v[j] = __fadd2_rn(v[j], v[j - 1]);
-                float2 inc = v[SW_R - 1];                        // inclusive scan of the thread totals across the warp
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
-                    const float ox = __shfl_up_sync(0xffffffffu, inc.x, d), oy = __shfl_up_sync(0xffffffffu, inc.y, d);
-                    if (lane >= d) { inc.x += ox; inc.y += oy; }
-                }
+                float2 inc = make_float2(0.f, 0.f), off = make_float2(0.f, 0.f);
                 float2 *tot = scan + 4 * (part & 1);
+                if (wact) {
+                    if (act) {
+                        const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
+                        const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
+                        v[0] = make_float2(a0.x, b0.x); v[1] = make_float2(a0.y, b0.y); v[2] = make_float2(a0.z, b0.z); v[3] = make_float2(a0.w, b0.w);
+                        v[4] = make_float2(a1.x, b1.x); v[5] = make_float2(a1.y, b1.y); v[6] = make_float2(a1.z, b1.z); v[7] = make_float2(a1.w, b1.w);
+#pragma unroll
+                        for (int j = 0; j < SW_R; ++j) {
+                            v[j] = __fadd2_rn(__fadd2_rn(v[j], mu_hi2), mu_lo2);
+                            Z[9 * g + j] = v[j];                 // zpad(8 g + j) = 9 g + j
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < SW_R; ++j) v[j] = make_float2(0.f, 0.f);
+                    }
+                    if (part == 0) {
+#pragma unroll
+                        for (int j = 0; j < SW_R; ++j) W[j] = v[j];
+                    }
+#pragma unroll
+                    for (int j = 1; j < SW_R; ++j) v[j] = __fadd2_rn(v[j], v[j - 1]);
+                    inc = v[SW_R - 1];                           // inclusive scan of the thread totals across the warp
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) {
+                        const float ox = __shfl_up_sync(0xffffffffu, inc.x, d), oy = __shfl_up_sync(0xffffffffu, inc.y, d);
+                        if (lane >= d) { inc.x += ox; inc.y += oy; }
+                    }
+                    // exclusive prefix inside the warp (no inc - total: -inf - -inf is NaN)
+                    off.x = __shfl_up_sync(0xffffffffu, inc.x, 1); off.y = __shfl_up_sync(0xffffffffu, inc.y, 1);
+                    if (lane == 0) off = make_float2(0.f, 0.f);
+                }
                 if (lane == 31) tot[wid] = inc;
-                float2 off;                                      // exclusive prefix inside the warp (no inc - total: -inf - -inf is NaN)
-                off.x = __shfl_up_sync(0xffffffffu, inc.x, 1); off.y = __shfl_up_sync(0xffffffffu, inc.y, 1);
-                if (lane == 0) off = make_float2(0.f, 0.f);
                 __syncthreads();                                 // totals visible; this part of raw is consumed, of Z written
                 if (part == nparts - 1 && tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);   // raw is free again
                 off = __fadd2_rn(off, carry);
