@@ -324,7 +324,6 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
             }
             if (tid == 0) P2[0] = make_float2(0.f, 0.f);
         }
-        __syncthreads();                           // P complete
 
         // ---- main loop: blocks of 8 widths, the running maximum ping-pongs between bestA and bestB ---------------------
         {
@@ -346,6 +345,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
             }
         }
         float2 (&best)[SW_R] = bestA;
+        __syncthreads();                           // P (written before the main loop) is complete for every warp
 
         // ---- width search inside the winning block, from the prefix sums: B_w(t) = P[t + w] - P[t] ------------------
         int wx[SW_R], wy[SW_R];
