@@ -3,6 +3,9 @@
 //
 //   B_N(t) = sum_{k<N} x[t+k];  SNR_N(t) = (B_N(t) - N mu) / sigma_N;  snr[t] = max_N, width[t] = smallest arg-max.
 //
+// Three kernels share one width loop (sweep8): boxcar_snr_sweep (planes, any nmax), boxcar_snr_sweep_narrow (planes,
+// nmax <= 24) and boxcar_search_fused (threshold in the kernel, no planes).
+//
 // Design (sm_100a; this is NOT the paper's one-thread-X-samples loop):
 //  * Persistent CTAs (one wave, grid = SMs x resident CTAs) walk the tiles; the raw samples of the NEXT tile are
 //    prefetched with cp.async (LDGSTS, 16 B) into shared memory while the current tile is swept.
@@ -10,26 +13,28 @@
 //    subtract, mu = mu_hi + mu_lo), so the inner loop is B += y; s = B * r_N with r_N = 1/sigma_N from a table.
 //  * One tile = 2048 consecutive samples of one row, as two sub-tiles A = [T0, T0+1024), B = [T0+1024, T0+2048).
 //    The working layout INTERLEAVES them, float2 Z[i] = (yA[i], yB[i]), so that one packed FADD2 / FMUL2
-//    (Blackwell packed fp32) advances one running sum of each sub-tile.  Measured on B200: a
-//    packed op holds the FMA pipe for two cycles but takes ONE issue slot, so the 3-input FMNMX of the running
-//    maximum and the arg-max bookkeeping (ALU pipe) issue in its shadow: the loop runs at the FMA-pipe floor of two
-//    lane-cycles per (sample, width) pair instead of the three issue slots of the scalar add / mul / max form.
+//    (Blackwell packed fp32) advances one running sum of each sub-tile.  Measured on B200: the
+//    loop is bound by instruction dispatch and register-operand bandwidth, not by a pipe; a packed op costs two
+//    dispatch clocks, like two scalar ones, but the packed mix is the fastest measured (about 10 % ahead of scalar),
+//    and r_N enters FMUL2 as a scalar-broadcast operand (one register read less than a (r, r) pair: 4-8 % faster).
 //  * Each thread owns 8 consecutive samples of each sub-tile and keeps a sliding window of 8 float2 in registers
 //    (the width loop is unrolled by 8, so the rotation is register renaming): one LDS.64 per width step.
 //  * Samples past the row end are staged as -inf: a running sum that has touched one is -inf for every wider
 //    width, so "only widths that fit" (reading A9) needs no masking in the loop.  Widths nmax < w <= 8 ceil(nmax/8)
 //    get a NaN reciprocal: FMNMX drops NaN operands, so they can never win and need no tail loop.
-//  * arg-max is deferred: the running maximum is advanced with 3-input FMNMX only, ping-ponging between two
-//    register sets so that the value before and after each block of 8 widths are both live; one compare + one
-//    select per block then record the block that last raised it.  After the loop that block alone is evaluated
-//    again, width by width, from a tile-local prefix sum P kept in shared memory (B_w(t) = P[t+w] - P[t], no
-//    dependency chain), and the smallest width attaining the block maximum is taken.  Blocks ascend and every
-//    comparison is a strict '>', so ties keep the smallest width (A7).  The SNR written is the running-sum value
-//    of the main loop; the prefix-sum re-evaluation only picks the width, and can differ from the running sums by
-//    fp32 rounding (~1e-6), i.e. only inside near-ties far below the 1e-3 tie tolerance.
+//  * arg-max of the general kernel is deferred: the running maximum is advanced with 3-input FMNMX only,
+//    ping-ponging between two register sets so that the value before and after each block of 8 widths are both
+//    live; one compare + one select per block then record the block that last raised it.  After the loop that block
+//    alone is evaluated again from a tile-local prefix sum P kept in shared memory (B_w(t) = P[t+w] - P[t], no
+//    dependency chain); the position inside the block rides in the 3 low mantissa bits of the 8 values (a larger tag
+//    is a smaller width), so one maximum gives the width.  Blocks ascend with a strict '>', so exact ties keep the
+//    smallest width (A7).  The SNR written is the running-sum value of the main loop; the re-evaluation only picks
+//    the width and differs from the running sums by fp32 rounding and the 3 tag bits (~1e-6 relative), i.e. only
+//    inside near-ties far below the 1e-3 tie tolerance.
 //
-// Roofline: 10 B/sample of HBM traffic (4 read + 4 snr + 2 width) against 2*Nmax fp32 lane-ops per sample on the
-// FMA pipe: FP32-pipe-bound for Nmax > ~28.
+// Roofline: 10 B/sample of HBM traffic (4 read + 4 snr + 2 width) against 3*Nmax fp32 lane-ops per sample (add,
+// multiply, compare) at one warp instruction per sub-partition per clock: FP32-issue-bound for Nmax > ~20
+// (DESIGN.md section 7).
 #include "spd_common.cuh"
 
 namespace spd {
@@ -55,7 +60,7 @@ struct SweepSmem {           // byte offsets into dynamic shared memory (all 16-
         z = 0;                                                           // float2 Z[zpad(SUB + H)]
         raw = z + round_up((zpad(SW_SUB + H) + 1) * 8, 16);              // float raw[TILE + H]
         p2 = raw + round_up((SW_TILE + H) * 4, 16);                      // float2 P[zpad(SUB + H + 1)]: prefix sums
-        scan = p2 + round_up((zpad(SW_SUB + H + 1) + 1) * 8, 16);        // float2 [2][4]: per-warp totals of the scan
+        scan = p2 + round_up((zpad(SW_SUB + H + 1) + 1) * 8, 16);        // float2 [2][4]: per-warp totals of the scan (double-buffered by part)
         rtf = scan + 64;                                                 // float r_w
         total = rtf + round_up(R * 4, 16);
     }
