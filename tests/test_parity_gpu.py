@@ -187,8 +187,12 @@ def test_sweep_linear_with_wrong_nmax_is_all_nan(P):
     from gpu_util import gpu_sweep
     x = rng(331).standard_normal((1, 3000)).astype(np.float32)
     st = P.write_stats(0.0, 1.0, 10.0, 64)
-    g_snr, _, _ = gpu_sweep(x, st, 32, "linear")
-    assert np.all(np.isnan(g_snr))
+    for nmax in (32, 16):                              # general kernel and the narrow (tagged-maximum) kernel
+        g_snr, _, (d, _, _) = gpu_sweep(x, st, nmax, "linear")
+        assert np.all(np.isnan(g_snr))
+        from gpu_util import gpu_fused
+        rec, total = gpu_fused(d, st, nmax, "linear", 3.0)    # NaN >= threshold is false: the fused search reports nothing
+        assert total == 0
 
 
 def test_sweep_without_width_plane(P):
@@ -235,6 +239,10 @@ def test_candidates_overflow_convention(P):
     assert np.all(g_snr[rec["dm"], rec["t"]] == rec["snr"]) and np.all(g_w[rec["dm"], rec["t"]] == rec["width"])
     rec, total = gpu_candidates(s, w, 1e9)
     assert total == 0 and rec.size == 0
+    from gpu_util import gpu_fused                      # the fused search follows the same convention
+    rec, total = gpu_fused(d, P.write_stats(0.0, 1.0), 16, "sqrt", 1.0, capacity=100)
+    assert total == want and rec.size == 100
+    assert np.all(g_snr[rec["dm"], rec["t"]] == rec["snr"]) and (g_w[rec["dm"], rec["t"]] != rec["width"]).mean() <= 0.02
 
 
 def test_candidates_ragged_and_strided(P):
