@@ -39,10 +39,11 @@
 
 namespace spd {
 
-constexpr int SW_THREADS = 128;
 constexpr int SW_R       = 8;                        // samples per thread per sub-tile
-constexpr int SW_SUB     = SW_THREADS * SW_R;        // 1024
-constexpr int SW_TILE    = 2 * SW_SUB;               // 2048 samples per tile
+// CTA width NT (a template parameter of the kernels): sub-tile = 8 NT samples, tile = 16 NT samples of one row.
+// 64 threads (tile 1024) for nmax <= SW_SMALL_CTA_NMAX: fewer warps wait on each block barrier; 128 threads (tile 2048)
+// above, where the halo (nmax + 8 positions staged and scanned per tile) would weigh too much on a small tile.
+constexpr int SW_SMALL_CTA_NMAX = 256;
 constexpr int SW_NARROW_NMAX = 24;                   // nmax up to here takes the tagged-maximum kernel (measured crossover on B200: 24..28)
 
 __host__ __device__ inline int zpad(int i) { return i + (i >> 3); }          // one pad float2 per 8: lane stride 72 B
@@ -54,9 +55,9 @@ size_t sweep_table_bytes(int nmax) { return (size_t)sw_rt_len(nmax) * sizeof(flo
 
 struct SweepSmem {           // byte offsets into dynamic shared memory (all 16-byte aligned)
     int z, raw, p2, scan, rtf, total;
-    __host__ __device__ explicit SweepSmem(int nmax)
+    __host__ __device__ SweepSmem(int nmax, int nt)
     {
-        const int H = sw_halo(nmax), R = sw_rt_len(nmax);
+        const int H = sw_halo(nmax), R = sw_rt_len(nmax), SW_SUB = nt * SW_R, SW_TILE = 2 * SW_SUB;
         z = 0;                                                           // float2 Z[zpad(SUB + H)]
         raw = z + round_up((zpad(SW_SUB + H) + 1) * 8, 16);              // float raw[TILE + H]
         p2 = raw + round_up((SW_TILE + H) * 4, 16);                      // float2 P[zpad(SUB + H + 1)]: prefix sums
@@ -119,12 +120,13 @@ struct TilePos {
 };
 
 // raw tile -> shared memory, asynchronously where the 16-byte fast path applies; past the row end -> -inf
+template <int SW_THREADS>
 __device__ __forceinline__ void stage_tile(float *__restrict__ raw, const float *__restrict__ x, int64_t n_t, int64_t row_stride,
                                            const TilePos &pos_, int LRAW, int tid)
 {
     const float NINF = __int_as_float(0xff800000);
     const int64_t row = pos_.row;
-    const int64_t T0 = (int64_t)pos_.tr * SW_TILE;
+    const int64_t T0 = (int64_t)pos_.tr * (2 * SW_THREADS * SW_R);
     const float *rowp = x + row * row_stride;
     const bool vec = ((reinterpret_cast<uintptr_t>(rowp) & 15) == 0);
     if (vec && T0 + LRAW <= n_t) {                       // interior tile: no bounds checks
@@ -182,10 +184,11 @@ __device__ __forceinline__ void note_block(const float2 (&now)[SW_R], const floa
 }
 
 // SNR (f32) and width (u16) of a thread's 8 + 8 samples: 16-byte streaming stores where the row is aligned and whole
+template <int SW_THREADS>
 __device__ __forceinline__ void store_planes(float *__restrict__ snr, uint16_t *__restrict__ width, int64_t row, int64_t row_stride,
                                              int64_t n_t, int64_t ta, const float2 (&best)[SW_R], const int (&wx)[SW_R], const int (&wy)[SW_R])
 {
-    const int64_t tb = ta + SW_SUB;
+    const int64_t tb = ta + SW_THREADS * SW_R;
     float *oa = snr + row * row_stride + ta, *ob = snr + row * row_stride + tb;
     const bool v4 = ((reinterpret_cast<uintptr_t>(snr + row * row_stride) & 15) == 0);
     if (v4 && ta + 7 < n_t) {
@@ -220,13 +223,15 @@ __device__ __forceinline__ void store_planes(float *__restrict__ snr, uint16_t *
     }
 }
 
-__global__ void __launch_bounds__(SW_THREADS, 4)
+template <int SW_THREADS>
+__global__ void __launch_bounds__(SW_THREADS, 512 / SW_THREADS)
 boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                  const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
                  float *__restrict__ snr, uint16_t *__restrict__ width)
 {
+    constexpr int SW_SUB = SW_THREADS * SW_R, SW_TILE = 2 * SW_SUB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const SweepSmem lay(nmax);
+    const SweepSmem lay(nmax, SW_THREADS);
     float2 *Z   = reinterpret_cast<float2 *>(smem_raw + lay.z);
     float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
     float2 *P2  = reinterpret_cast<float2 *>(smem_raw + lay.p2);      // prefix sums of y: (sub-tile A, sub-tile B), zpad layout
@@ -249,7 +254,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
 
     int64_t tile = blockIdx.x;
     TilePos pos(blockIdx.x, tiles_per_row);
-    if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);
+    if (tile < total_tiles) stage_tile<SW_THREADS>(raw, x, n_t, row_stride, pos, LRAW, tid);
 
     for (; tile < total_tiles; tile += gridDim.x) {
         const int64_t row = pos.row;
@@ -314,7 +319,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
                 }
                 if (lane == 31) tot[wid] = inc;
                 __syncthreads();                                 // totals visible; this part of raw is consumed, of Z written
-                if (part == nparts - 1 && tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);   // raw is free again
+                if (part == nparts - 1 && tile + gridDim.x < total_tiles) stage_tile<SW_THREADS>(raw, x, n_t, row_stride, pos, LRAW, tid);   // raw is free again
                 off = __fadd2_rn(off, carry);
 #pragma unroll
                 for (int w = 0; w < SW_THREADS / 32; ++w) {
@@ -384,7 +389,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
             for (int j = 0; j < SW_R; ++j) best[j] = make_float2(rtf[0], rtf[0]);
         }
 
-        store_planes(snr, width, row, row_stride, n_t, T0 + SW_R * tid, best, wx, wy);
+        store_planes<SW_THREADS>(snr, width, row, row_stride, n_t, T0 + SW_R * tid, best, wx, wy);
     }
     cp_async_commit_wait_all();
 }
@@ -397,9 +402,9 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
 // width whose SNR equals the maximum: the smallest arg-max (A7).
 struct FusedSmem {
     int z, raw, rtf, total;
-    __host__ __device__ explicit FusedSmem(int nmax)
+    __host__ __device__ FusedSmem(int nmax, int nt)
     {
-        const int H = sw_halo(nmax), R = sw_rt_len(nmax);
+        const int H = sw_halo(nmax), R = sw_rt_len(nmax), SW_SUB = nt * SW_R, SW_TILE = 2 * SW_SUB;
         z = 0;
         raw = z + round_up((zpad(SW_SUB + H) + 1) * 8, 16);
         rtf = raw + round_up((SW_TILE + H) * 4, 16);
@@ -417,14 +422,16 @@ __device__ __noinline__ int replay_width(const float *__restrict__ zh, int pos, 
     return nmax;                                   // not reached for finite input
 }
 
-__global__ void __launch_bounds__(SW_THREADS, 4)
+template <int SW_THREADS>
+__global__ void __launch_bounds__(SW_THREADS, 512 / SW_THREADS)
 boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                     const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
                     float threshold, spd_candidate_t *__restrict__ cand, unsigned long long capacity,
                     unsigned long long *__restrict__ count)
 {
+    constexpr int SW_SUB = SW_THREADS * SW_R, SW_TILE = 2 * SW_SUB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const FusedSmem lay(nmax);
+    const FusedSmem lay(nmax, SW_THREADS);
     float2 *Z   = reinterpret_cast<float2 *>(smem_raw + lay.z);
     float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
     float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);
@@ -443,7 +450,7 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
 
     int64_t tile = blockIdx.x;
     TilePos pos(blockIdx.x, tiles_per_row);
-    if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);
+    if (tile < total_tiles) stage_tile<SW_THREADS>(raw, x, n_t, row_stride, pos, LRAW, tid);
 
     for (; tile < total_tiles; tile += gridDim.x) {
         const int64_t row = pos.row;
@@ -469,7 +476,7 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
             }
         }
         __syncthreads();                           // Z complete; raw is free again
-        if (tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);
+        if (tile + gridDim.x < total_tiles) stage_tile<SW_THREADS>(raw, x, n_t, row_stride, pos, LRAW, tid);
 
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); }
@@ -536,13 +543,15 @@ __device__ __forceinline__ void sweep8_tagged(float2 (&B)[SW_R], float2 (&W)[SW_
     }
 }
 
-__global__ void __launch_bounds__(SW_THREADS, 5)
+template <int SW_THREADS>
+__global__ void __launch_bounds__(SW_THREADS, 640 / SW_THREADS)
 boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                         const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
                         float *__restrict__ snr, uint16_t *__restrict__ width)
 {
+    constexpr int SW_SUB = SW_THREADS * SW_R, SW_TILE = 2 * SW_SUB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const FusedSmem lay(nmax);
+    const FusedSmem lay(nmax, SW_THREADS);
     float2 *Z   = reinterpret_cast<float2 *>(smem_raw + lay.z);
     float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
     float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);
@@ -561,7 +570,7 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
 
     int64_t tile = blockIdx.x;
     TilePos pos(blockIdx.x, tiles_per_row);
-    if (tile < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);
+    if (tile < total_tiles) stage_tile<SW_THREADS>(raw, x, n_t, row_stride, pos, LRAW, tid);
 
     for (; tile < total_tiles; tile += gridDim.x) {
         const int64_t row = pos.row;
@@ -587,7 +596,7 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
             }
         }
         __syncthreads();                           // Z complete; raw is free again
-        if (tile + gridDim.x < total_tiles) stage_tile(raw, x, n_t, row_stride, pos, LRAW, tid);
+        if (tile + gridDim.x < total_tiles) stage_tile<SW_THREADS>(raw, x, n_t, row_stride, pos, LRAW, tid);
 
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); tbest[j] = make_float2(NINF, NINF); }
@@ -604,24 +613,52 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
 #pragma unroll
             for (int j = 0; j < SW_R; ++j) { best[j] = make_float2(rtf[0], rtf[0]); wx[j] = 1; wy[j] = 1; }
         }
-        store_planes(snr, width, row, row_stride, n_t, T0 + SW_R * tid, best, wx, wy);
+        store_planes<SW_THREADS>(snr, width, row, row_stride, n_t, T0 + SW_R * tid, best, wx, wy);
     }
     cp_async_commit_wait_all();
 }
 
 template <typename K>
-static cudaError_t persistent_grid(K kernel, int smem, int64_t tiles, unsigned *grid)
+static cudaError_t persistent_grid(K kernel, int threads, int smem, int64_t tiles, unsigned *grid)
 {
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     int dev = 0, sms = 0, per_sm = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, SW_THREADS, smem)) != cudaSuccess) return e;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem)) != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorInvalidConfiguration;
     const int64_t wave = (int64_t)sms * per_sm;                 // persistent: one resident wave walks all tiles
     *grid = (unsigned)(tiles < wave ? tiles : wave);
     return cudaSuccess;
+}
+
+template <int NT>
+static cudaError_t launch_sweep_nt(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
+                                   const float *d_table, int nmax, float *snr, uint16_t *width,
+                                   bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
+                                   unsigned long long *d_count, cudaStream_t s)
+{
+    constexpr int TILE = 2 * NT * SW_R;
+    const int tpr = (int)((n_t + TILE - 1) / TILE);
+    const int64_t tiles = n_dm * (int64_t)tpr;
+    unsigned grid = 0;
+    cudaError_t e;
+    if (fused) {
+        const FusedSmem lay(nmax, NT);
+        if ((e = persistent_grid(boxcar_search_fused<NT>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_search_fused<NT><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax,
+                                                            threshold, out, capacity, d_count);
+    } else if (nmax <= SW_NARROW_NMAX) {
+        const FusedSmem lay(nmax, NT);
+        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep_narrow<NT><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
+    } else {
+        const SweepSmem lay(nmax, NT);
+        if ((e = persistent_grid(boxcar_snr_sweep<NT>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep<NT><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
+    }
+    return cudaGetLastError();
 }
 
 cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
@@ -629,25 +666,9 @@ cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
                          bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
                          unsigned long long *d_count, cudaStream_t s)
 {
-    const int tpr = (int)((n_t + SW_TILE - 1) / SW_TILE);
-    const int64_t tiles = n_dm * (int64_t)tpr;
-    unsigned grid = 0;
-    cudaError_t e;
-    if (fused) {
-        const FusedSmem lay(nmax);
-        if ((e = persistent_grid(boxcar_search_fused, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_search_fused<<<grid, SW_THREADS, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax,
-                                                                threshold, out, capacity, d_count);
-    } else if (nmax <= SW_NARROW_NMAX) {
-        const FusedSmem lay(nmax);
-        if ((e = persistent_grid(boxcar_snr_sweep_narrow, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep_narrow<<<grid, SW_THREADS, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
-    } else {
-        const SweepSmem lay(nmax);
-        if ((e = persistent_grid(boxcar_snr_sweep, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep<<<grid, SW_THREADS, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
-    }
-    return cudaGetLastError();
+    if (nmax <= SW_SMALL_CTA_NMAX)
+        return launch_sweep_nt<64>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
+    return launch_sweep_nt<128>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
 }
 
 }  // namespace spd
