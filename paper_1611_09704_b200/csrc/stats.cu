@@ -176,13 +176,27 @@ stats_boxcar_partial(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int
                 }
             }
         }
+        if (__all_sync(0xffffffffu, t.m == (double)SB_WIN)) {
+            // every run is full: eq. 2 for equal sizes m, S = S1 + S2 + (T1 - T2)^2 / (2m), with 1/(2m) a constant
+            // per level (no fp64 division); the order of the two operands is that of the general path below
 #pragma unroll
-        for (int lvl = 0; lvl < 5; ++lvl) {
-            Tri o;
-            o.m = __shfl_xor_sync(0xffffffffu, t.m, 1 << lvl);
-            o.T = __shfl_xor_sync(0xffffffffu, t.T, 1 << lvl);
-            o.S = __shfl_xor_sync(0xffffffffu, t.S, 1 << lvl);
-            if ((lane >> lvl) & 1) { Tri a = o; tri_merge(a, t); t = a; } else tri_merge(t, o);
+            for (int lvl = 0; lvl < 5; ++lvl) {
+                const double T2 = __shfl_xor_sync(0xffffffffu, t.T, 1 << lvl);
+                const double S2 = __shfl_xor_sync(0xffffffffu, t.S, 1 << lvl);
+                const double d = t.T - T2;
+                t.S = (t.S + S2) + d * d * (1.0 / (double)(2 * (SB_WIN << lvl)));
+                t.T += T2;
+            }
+            t.m = (double)(32 * SB_WIN);
+        } else {
+#pragma unroll
+            for (int lvl = 0; lvl < 5; ++lvl) {
+                Tri o;
+                o.m = __shfl_xor_sync(0xffffffffu, t.m, 1 << lvl);
+                o.T = __shfl_xor_sync(0xffffffffu, t.T, 1 << lvl);
+                o.S = __shfl_xor_sync(0xffffffffu, t.S, 1 << lvl);
+                if ((lane >> lvl) & 1) { Tri a = o; tri_merge(a, t); t = a; } else tri_merge(t, o);
+            }
         }
         if (lane == 0) tri_merge(acc, t);
     }
