@@ -29,8 +29,8 @@ import gen  # noqa: E402
 METRIC = "DM×time samples/s through boxcar SNR search (×real-time); HBM GB/s vs peak"
 SM_COUNT, FP32_LANES_PER_SM = 148, 128
 OPS_PER_PAIR = 3.0      # fp32 add + fp32 multiply + compare per (sample, width) pair
-# DRAM bytes per launch of boxcar_snr_sweep on config 3 from `ncu --set full` (profiles/r01e_sweep_c3.md): read + write
-SWEEP_DRAM_TRAFFIC_C3 = 6.305278e9 + 9.384107e9
+# DRAM bytes per launch of boxcar_snr_sweep on config 3 from `ncu --set full` (profiles/r01f_sweep_c3.md): read + write
+SWEEP_DRAM_TRAFFIC_C3 = 6.324072e9 + 9.386170e9
 
 
 def _peaks():
