@@ -156,6 +156,8 @@ def run_ours(args):
     import torch.distributed as dist
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    from paper_1611_09704_b200 import build as _build
+    _build.ensure_built()                      # a fresh clone has no libspd.so (git-ignored); nvcc is in the image
     import paper_1611_09704_b200 as P
     P.lib()
 

@@ -41,5 +41,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def ensure_built() -> str:
+    """Build libspd.so if it is not there at all (a fresh clone: built artefacts are git-ignored).  Callers that time
+    or test the library use this; the library itself never builds or falls back (binding.lib() raises)."""
+    return LIB if os.path.exists(LIB) else build(force=True)
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

@@ -19,6 +19,8 @@ def P():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     import paper_1611_09704_b200 as P
+    from paper_1611_09704_b200 import build as B
+    B.ensure_built()
     P.lib()
     return P
 

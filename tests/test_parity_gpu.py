@@ -22,6 +22,8 @@ def P():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     import paper_1611_09704_b200 as P
+    from paper_1611_09704_b200 import build as B
+    B.ensure_built()
     P.lib()      # fails loudly when libspd.so is missing
     return P
 
