@@ -1,6 +1,7 @@
 """spd-b200: single-pulse detection (arXiv 1611.09704) as hand-written sm_100a CUDA kernels behind a C ABI.
 
-`binding` is a thin ctypes layer over libspd.so (include/spd.h); `build` compiles the library in-tree.
+`binding` is a thin ctypes layer over libspd.so (include/spd.h); `build` compiles the library in-tree; `shard`
+(DM-row sharding over torch.distributed) and `stream` (copy / compute overlap over consecutive chunks) are plumbing.
 Nothing here computes on the CPU; the package is independent of the CPU checker used by the tests.
 """
 from .binding import (  # noqa: F401

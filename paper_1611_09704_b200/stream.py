@@ -1,0 +1,99 @@
+"""Chunked streaming with copy / compute overlap (the real-time pipeline shape of PAPER.md:97).
+
+A telescope back-end produces one de-dispersed chunk [n_dm][n_t] after another.  `ChunkStream` keeps `depth` device
+slots; the host-to-device copy of chunk i+1 runs on a copy stream while spd_stats + spd_search_fused of chunk i run on
+a compute stream, and the statistics, the hit count and the records of a finished chunk come back through pinned host
+buffers.  This module is plumbing only (CUDA streams and events from PyTorch, argument marshalling); every step of
+the search runs in the kernels behind the C ABI.
+
+Chunks along TIME for the same DM trials must overlap by Nmax - 1 samples on the caller's side: the last Nmax - 1
+samples of a row see only the widths that fit (reading A9), so the next chunk starts Nmax - 1 samples
+before the end of this one and the caller drops the records of the overlap it has already seen.
+"""
+from __future__ import annotations
+
+from typing import List, Optional, Tuple
+
+import numpy as np
+import torch
+
+from . import binding as B
+
+
+class ChunkStream:
+    def __init__(self, n_dm: int, n_t: int, nmax: int, mode="sqrt", threshold: float = 6.0, capacity: int = 1 << 20,
+                 depth: int = 2, device="cuda"):
+        if depth < 1:
+            raise ValueError("depth >= 1")
+        B.lib()
+        self.n_dm, self.n_t, self.nmax, self.mode, self.threshold, self.capacity = n_dm, n_t, int(nmax), mode, float(threshold), int(capacity)
+        self.dev = torch.device(device)
+        self.copy_stream = torch.cuda.Stream(self.dev)
+        self.compute_stream = torch.cuda.Stream(self.dev)
+        self.nsig = self.nmax if B._MODES[mode] != 0 else 0
+        self.slots = []
+        for _ in range(depth):
+            out, cnt = B.new_candidates(self.capacity, self.dev)
+            self.slots.append({
+                "x": torch.empty((n_dm, n_t), dtype=torch.float32, device=self.dev),
+                "stats": B.new_stats(self.dev), "ws": B.new_workspace(n_dm, n_t, self.nmax, self.dev),
+                "out": out, "cnt": cnt,
+                "h_out": torch.zeros((self.capacity, 4), dtype=torch.int32).pin_memory(),
+                "h_cnt": torch.zeros(1, dtype=torch.int64).pin_memory(),
+                "h_stats": torch.zeros(B.STATS_BYTES, dtype=torch.uint8).pin_memory(),
+                "copied": torch.cuda.Event(), "done": torch.cuda.Event(), "busy": False,
+            })
+        self.next_slot = 0
+        self.bytes_h2d = n_dm * n_t * 4
+
+    def submit(self, h_x: torch.Tensor) -> int:
+        """Enqueue one chunk (a pinned CPU float32 [n_dm][n_t] tensor makes the copy asynchronous); returns a ticket.
+        The slot's previous result must have been collected."""
+        if h_x.is_cuda or h_x.dtype != torch.float32 or tuple(h_x.shape) != (self.n_dm, self.n_t) or not h_x.is_contiguous():
+            raise B.SpdError("h_x must be a contiguous CPU float32 [n_dm][n_t] tensor of the stream's shape")
+        k = self.next_slot
+        s = self.slots[k]
+        if s["busy"]:
+            raise B.SpdError("ChunkStream: collect the result of the oldest chunk before submitting another")
+        self.next_slot = (k + 1) % len(self.slots)
+        with torch.cuda.stream(self.copy_stream):
+            s["x"].copy_(h_x, non_blocking=True)
+            s["copied"].record(self.copy_stream)
+        with torch.cuda.stream(self.compute_stream):
+            self.compute_stream.wait_event(s["copied"])
+            B.spd_stats(s["x"], self.nsig, s["stats"], s["ws"], stream=self.compute_stream)
+            B.spd_search_fused(s["x"], s["stats"], self.nmax, self.mode, self.threshold, s["out"], s["cnt"], ws=s["ws"],
+                               stream=self.compute_stream)
+            s["h_cnt"].copy_(s["cnt"], non_blocking=True)
+            s["h_stats"].copy_(s["stats"], non_blocking=True)
+            s["h_out"].copy_(s["out"], non_blocking=True)          # whole buffer: the count is not known on the host yet
+            s["done"].record(self.compute_stream)
+        s["busy"] = True
+        return k
+
+    def result(self, ticket: int) -> Tuple[np.ndarray, int, np.ndarray]:
+        """Wait for a chunk: (records written, total hit count, statistics).  The arrays are views of the slot's pinned
+        buffers and are overwritten when the slot is reused."""
+        s = self.slots[ticket]
+        if not s["busy"]:
+            raise B.SpdError("ChunkStream: no chunk in flight in this slot")
+        s["done"].synchronize()
+        s["busy"] = False
+        total = int(s["h_cnt"][0])
+        got = min(total, self.capacity)
+        rec = s["h_out"][:got].numpy().view(B.CAND_DTYPE).reshape(-1)
+        return rec, total, s["h_stats"].numpy().view(B.STATS_DTYPE)
+
+    def run(self, chunks: List[torch.Tensor]) -> List[Tuple[np.ndarray, int]]:
+        """Convenience: push a list of chunks through the pipeline in order; returns copies of (records, count)."""
+        res: List[Optional[Tuple[np.ndarray, int]]] = []
+        tickets: List[int] = []
+        for h in chunks:
+            if len(tickets) == len(self.slots):
+                rec, total, _ = self.result(tickets.pop(0))
+                res.append((rec.copy(), total))
+            tickets.append(self.submit(h))
+        for t in tickets:
+            rec, total, _ = self.result(t)
+            res.append((rec.copy(), total))
+        return res
