@@ -114,7 +114,7 @@ UNIT = O.Stats(0, 0.0, 0.0, 0.0, 1.0)
 @pytest.mark.parametrize("n_dm,n_t,nmax", [
     (1, 1, 1), (1, 7, 1), (1, 7, 7), (3, 100, 8), (2, 100, 5), (2, 100, 13), (1, 1023, 16), (1, 1024, 32),
     (1, 1025, 32), (2, 2047, 24), (2, 2048, 64), (3, 2049, 100), (2, 5000, 128), (1, 4097, 7), (5, 3000, 512),
-    (2, 600, 600), (1, 9001, 1000),
+    (2, 600, 600), (1, 9001, 1000), (1, 9000, 4096), (2, 4096, 4096),      # the last two: the API's maximum nmax
 ])
 def test_sweep_integer_data_forced_stats(P, n_dm, n_t, nmax):
     # small integers: every running sum is exact in fp32 and fp64 (pin P6 on the GPU side)
