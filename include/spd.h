@@ -102,7 +102,9 @@ spd_status spd_candidates(const float *d_snr, const uint16_t *d_width, int64_t n
 
 /* Steps 2-4 fused: the sweep of spd_boxcar_snr with the threshold of spd_candidates applied in the
  * same kernel; the SNR / width planes are never written (the list is the only downstream product,
- * PAPER.md:93).  Same records as spd_boxcar_snr + spd_candidates. */
+ * PAPER.md:93).  Same (dm, t, snr) as spd_boxcar_snr + spd_candidates, bit for bit; the width of a hit is found by
+ * replaying its running sums, so it is the exact smallest arg-max of the fp32 values and can differ from the plane
+ * path's width only inside the near-ties described there.  *d_count / capacity follow spd_candidates. */
 spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
                             const spd_stats_t *d_stats, int nmax, spd_sigma_mode mode, float threshold,
                             spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,
