@@ -403,3 +403,35 @@ def test_argument_errors_on_device(P):
         P.spd_stats(x, 5000)
     with pytest.raises(P.SpdError):
         P.spd_boxcar_snr(x, st, 8, ws=torch.empty(16, dtype=torch.uint8, device="cuda"))   # SPD_ERR_WORKSPACE
+
+
+def test_three_call_path_is_cuda_graph_capturable(P):
+    """Every call only enqueues work on the caller's stream and keeps no state, so a step can be captured once and
+    replayed (config 1 is launch-latency-bound: DESIGN.md section 8)."""
+    cfg = gen.get_config(1)
+    x = torch.from_numpy(gen.make_array(cfg)).cuda()
+    st, ws = P.new_stats("cuda"), P.new_workspace(cfg.n_dm, cfg.n_t, 32, "cuda")
+    snr = torch.empty_like(x)
+    w = torch.empty(x.shape, dtype=torch.uint16, device="cuda")
+    out, cnt = P.new_candidates(4096, "cuda")
+
+    def step():
+        P.spd_stats(x, 0, st, ws)
+        P.spd_boxcar_snr(x, st, 32, "sqrt", snr, w, ws)
+        P.spd_candidates(snr, w, cfg.threshold, out, cnt)
+
+    step()
+    torch.cuda.synchronize()
+    ref = (snr.clone(), w.view(torch.int16).clone(), int(cnt.item()), st.clone())
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        step()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            step()
+    torch.cuda.synchronize()
+    snr.zero_(); cnt.zero_(); st.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(snr, ref[0]) and torch.equal(w.view(torch.int16), ref[1]) and int(cnt.item()) == ref[2] > 0
+    assert torch.equal(st, ref[3])
