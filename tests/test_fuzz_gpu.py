@@ -57,9 +57,9 @@ def test_random_cases_against_the_oracle(P, seed):
         r = CMP.compare_planes(x, o.mean, sig, snr.cpu().numpy(), width.cpu().numpy(), o_snr, o_w, o_m)
         assert r, tag + " " + str(r)
         rec, total = gpu_candidates(snr, width, thr, capacity=1 << 18)
-        r = CMP.compare_candidates(rec["dm"], rec["t"], rec["snr"], rec["width"], total, 1 << 18, o_snr, o_w, o_m, thr)
+        r = CMP.compare_candidates(rec["dm"], rec["t"], rec["snr"], rec["width"], total, 1 << 18, o_snr, o_w, o_m, thr, x, o.mean, sig)
         assert r, tag + " " + str(r)
         rec2, total2 = gpu_fused(d, st, nmax, mode, thr, capacity=1 << 18)
-        r = CMP.compare_candidates(rec2["dm"], rec2["t"], rec2["snr"], rec2["width"], total2, 1 << 18, o_snr, o_w, o_m, thr)
+        r = CMP.compare_candidates(rec2["dm"], rec2["t"], rec2["snr"], rec2["width"], total2, 1 << 18, o_snr, o_w, o_m, thr, x, o.mean, sig)
         assert r and total2 == total, tag + " " + str(r)
         done += 1

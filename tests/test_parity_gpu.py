@@ -219,7 +219,7 @@ def test_candidates_threshold_inclusive_and_set_equality(P):
     for thr in (10.0, 6.0, 3.0):
         rec, total = gpu_candidates(s, w, thr)
         assert total == int((g_snr >= np.float32(thr)).sum())
-        r = CMP.compare_candidates(rec["dm"], rec["t"], rec["snr"], rec["width"], total, 1 << 16, o_snr, o_w, o_m, thr)
+        r = CMP.compare_candidates(rec["dm"], rec["t"], rec["snr"], rec["width"], total, 1 << 16, o_snr, o_w, o_m, thr, x, 0.0, sig)
         assert r, str(r)
         rec2, total2 = gpu_fused(d, st, 8, "sqrt", thr)
         assert total2 == total
@@ -291,7 +291,7 @@ def _whole_path(P, cfg, x, nmax, rows=None, fused=True):
     m = np.isin(rec["dm"], sel)
     dm_local = np.array([pos[int(v)] for v in rec["dm"][m]], dtype=np.int64)
     rc = CMP.compare_candidates(dm_local, rec["t"][m], rec["snr"][m], rec["width"][m], int(m.sum()), 1 << 22,
-                                o_snr, o_w, o_m, cfg.threshold)
+                                o_snr, o_w, o_m, cfg.threshold, xs, o.mean, sig)
     assert rc, str(rc)
     if fused:
         # the fused kernel takes the width by replaying the running sums, the plane kernel from a prefix sum: the
@@ -305,7 +305,7 @@ def _whole_path(P, cfg, x, nmax, rows=None, fused=True):
         m2 = np.isin(rec2["dm"], sel)
         dm2 = np.array([pos[int(v)] for v in rec2["dm"][m2]], dtype=np.int64)
         rc2 = CMP.compare_candidates(dm2, rec2["t"][m2], rec2["snr"][m2], rec2["width"][m2], int(m2.sum()), 1 << 22,
-                                     o_snr, o_w, o_m, cfg.threshold)
+                                     o_snr, o_w, o_m, cfg.threshold, xs, o.mean, sig)
         assert rc2, str(rc2)
     return rec, total, r, rc
 
