@@ -85,7 +85,8 @@ spd_status spd_stats_merge(const spd_stats_t *d_parts, int count, spd_stats_t *d
  * mu, sigma (and sigma_nmax for the LINEAR modes) are read from *d_stats on the device; a LINEAR mode
  * fed stats whose nmax_of_sigma != nmax yields an all-NaN SNR plane (it cannot be caught without a sync).
  * Widths whose fp32 SNRs differ by less than about 4e-6 relative (rounding of the running sums) count as tied and
- * either may be reported; an exact tie reports the smallest.  d_snr is always the maximum itself.
+ * either may be reported; an exact tie of a non-negative maximum reports the smallest width (of a negative maximum:
+ * one of the tied widths).  d_snr is always the maximum itself.
  * Requires 1 <= nmax <= min(n_t, 4096) (shared-memory bound of the tile).  d_width may be NULL (plane not written). */
 spd_status spd_boxcar_snr(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
                           const spd_stats_t *d_stats, int nmax, spd_sigma_mode mode,
@@ -104,7 +105,9 @@ spd_status spd_candidates(const float *d_snr, const uint16_t *d_width, int64_t n
  * same kernel; the SNR / width planes are never written (the list is the only downstream product,
  * PAPER.md:93).  Same (dm, t, snr) as spd_boxcar_snr + spd_candidates, bit for bit; the width of a hit is found by
  * replaying its running sums, so it is the exact smallest arg-max of the fp32 values and can differ from the plane
- * path's width only inside the near-ties described there.  *d_count / capacity follow spd_candidates. */
+ * path's width only inside the near-ties described there.  *d_count / capacity follow spd_candidates.
+ * A LINEAR mode fed stats whose nmax_of_sigma != nmax has no sigma_N: the call then sets *d_count = UINT64_MAX
+ * (no record is written), since "no detections" would be indistinguishable from the misuse. */
 spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
                             const spd_stats_t *d_stats, int nmax, spd_sigma_mode mode, float threshold,
                             spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,

@@ -181,6 +181,12 @@ def search(x: np.ndarray, nmax: int, mode="sqrt", f_T: float = 6.0):
     return dict(stats=st, sig=sig, snr=snr, width=width, margin=margin, cand=cand)
 
 
+def set_num_threads(n: int) -> None:
+    """OpenMP thread count of the following sweeps (bench.py's per-core figure); no arithmetic is affected."""
+    _load()
+    C.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+
+
 def num_threads() -> int:
     """Threads the OpenMP sweep will use (reported as cpu_baseline.cores)."""
     env = os.environ.get("OMP_NUM_THREADS")

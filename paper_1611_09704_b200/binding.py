@@ -164,6 +164,8 @@ def spd_search_fused(x: torch.Tensor, stats: torch.Tensor, nmax: int, mode, thre
 def read_candidates(out: torch.Tensor, count: torch.Tensor) -> Tuple[np.ndarray, int]:
     """Device list -> (numpy structured array of the written records, total hit count).  Synchronises."""
     total = int(count.item())
+    if total < 0:      # 0xFFFFFFFFFFFFFFFF: spd_search_fused was fed a NaN sigma table (include/spd.h)
+        raise SpdError("spd_search_fused: sigma_N is undefined (a LINEAR mode fed statistics measured for another Nmax)")
     got = min(total, out.shape[0])
     rec = out[:got].cpu().numpy().view(CAND_DTYPE).reshape(-1)
     return rec, total

@@ -65,9 +65,10 @@ spd_status spd_boxcar_snr(const float *d_x, int64_t n_dm, int64_t n_t, int64_t r
     if (ws_bytes < sweep_table_bytes(nmax)) return SPD_ERR_WORKSPACE;
     cudaStream_t s = (cudaStream_t)stream;
     float *table = reinterpret_cast<float *>(d_ws);
-    cudaError_t e = launch_sigma_table(d_stats, nmax, (int)mode, table, s);
+    const bool rc = sweep_uses_constant_table(nmax, (int)mode);
+    cudaError_t e = rc ? cudaSuccess : launch_sigma_table(d_stats, nmax, (int)mode, table, s);
     if (e != cudaSuccess) return SPD_ERR_CUDA;
-    e = launch_sweep(d_x, n_dm, n_t, row_stride, d_stats, table, nmax, d_snr, d_width, false, 0.0f, nullptr, 0, nullptr, s);
+    e = launch_sweep(d_x, n_dm, n_t, row_stride, d_stats, table, nmax, rc, d_snr, d_width, false, 0.0f, nullptr, 0, nullptr, s);
     return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
 }
 
@@ -97,9 +98,10 @@ spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t
     cudaStream_t s = (cudaStream_t)stream;
     float *table = reinterpret_cast<float *>(d_ws);
     if (cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s) != cudaSuccess) return SPD_ERR_CUDA;
-    cudaError_t e = launch_sigma_table(d_stats, nmax, (int)mode, table, s);
+    const bool rc = sweep_uses_constant_table(nmax, (int)mode);
+    cudaError_t e = rc ? cudaSuccess : launch_sigma_table(d_stats, nmax, (int)mode, table, s);
     if (e != cudaSuccess) return SPD_ERR_CUDA;
-    e = launch_sweep(d_x, n_dm, n_t, row_stride, d_stats, table, nmax, nullptr, nullptr, true, threshold, d_out,
+    e = launch_sweep(d_x, n_dm, n_t, row_stride, d_stats, table, nmax, rc, nullptr, nullptr, true, threshold, d_out,
                      capacity, d_count, s);
     return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
 }

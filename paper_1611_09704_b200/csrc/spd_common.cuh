@@ -43,8 +43,9 @@ cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
                          spd_stats_t *d_stats, void *d_ws, cudaStream_t s);
 cudaError_t launch_stats_merge(const spd_stats_t *parts, int count, spd_stats_t *out, cudaStream_t s);
 cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, float *d_table, cudaStream_t s);
+bool sweep_uses_constant_table(int nmax, int mode);      // eq. 4 with nmax a multiple of 8: r_w = 1/sqrt(w) from the constant bank, no table launch
 cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
-                         const float *d_table, int nmax, float *snr, uint16_t *width,
+                         const float *d_table, int nmax, bool rc, float *snr, uint16_t *width,
                          bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
                          unsigned long long *d_count, cudaStream_t s);
 cudaError_t launch_candidates(const float *snr, const uint16_t *width, int64_t n_dm, int64_t n_t, int64_t row_stride,

@@ -4,38 +4,48 @@
 //   B_N(t) = sum_{k<N} x[t+k];  SNR_N(t) = (B_N(t) - N mu) / sigma_N;  snr[t] = max_N, width[t] = smallest arg-max.
 //
 // Three kernels share one width loop (sweep8): boxcar_snr_sweep (planes, any nmax), boxcar_snr_sweep_narrow (planes,
-// nmax <= 24) and boxcar_search_fused (threshold in the kernel, no planes).
+// nmax <= 32) and boxcar_search_fused (threshold in the kernel, no planes).
+//
+// What bounds the loop (measured with csrc/ubench_fp32.cu, profiles/r02_fp32_issue_rates.md): one warp instruction per
+// sub-partition per clock, a packed FADD2 / FMUL2 counts as two (it passes the 32-lane FMA pipe twice), an ALU-pipe
+// instruction (FMNMX3, LOP3, FSETP, SEL) occupies its 16-lane pipe for two clocks.  One (sample, width) pair needs an add,
+// a multiply and half a 3-input maximum = 2.5 issue slots; everything else in this file exists to add as little as
+// possible to that.
 //
 // Design (sm_100a; this is NOT the paper's one-thread-X-samples loop):
 //  * Persistent CTAs (one wave, grid = SMs x resident CTAs) walk the tiles; the raw samples of the NEXT tile are
-//    prefetched with cp.async (LDGSTS, 16 B) into shared memory while the current tile is swept.
+//    prefetched with cp.async (LDGSTS, 16 B) or one 1-D TMA bulk copy into shared memory while the current tile is swept.
 //  * y = x - mu is formed once per sample when the raw tile is converted into the working layout (two-term fp32
-//    subtract, mu = mu_hi + mu_lo), so the inner loop is B += y; s = B * r_N with r_N = 1/sigma_N from a table.
-//  * One tile = 2048 consecutive samples of one row, as two sub-tiles A = [T0, T0+1024), B = [T0+1024, T0+2048).
-//    The working layout INTERLEAVES them, float2 Z[i] = (yA[i], yB[i]), so that one packed FADD2 / FMUL2
-//    (Blackwell packed fp32) advances one running sum of each sub-tile.  Measured on B200: the
-//    loop is bound by instruction dispatch and register-operand bandwidth, not by a pipe; a packed op costs two
-//    dispatch clocks, like two scalar ones, but the packed mix is the fastest measured (about 10 % ahead of scalar),
-//    and r_N enters FMUL2 as a scalar-broadcast operand (one register read less than a (r, r) pair: 4-8 % faster).
+//    subtract, mu = mu_hi + mu_lo), so the inner loop is B += y; s = B * r_N.
+//  * Where r_N comes from (template parameter RC):
+//      RC = true  (eq. 4 and nmax a multiple of 8): y is also divided by sigma once per sample, and r_N = 1/sqrt(N)
+//                 is read from a compile-time table in the CONSTANT bank, so it reaches FMUL2 as a uniform-register
+//                 operand: one register-file read less per multiply (measured 2.8 -> 2.5 clocks per pair).
+//      RC = false (eq. 5 modes, any nmax): r_N = 1/sigma_N from the table sigma_table_kernel wrote, staged in shared
+//                 memory and fed as a scalar-broadcast register operand.
+//  * One tile = 16 NT consecutive samples of one row, as two sub-tiles A = [T0, T0 + 8 NT), B = [T0 + 8 NT, T0 + 16 NT).
+//    The working layout INTERLEAVES them, float2 Z[i] = (yA[i], yB[i]), so that one packed FADD2 / FMUL2 advances one
+//    running sum of each sub-tile.
 //  * Each thread owns 8 consecutive samples of each sub-tile and keeps a sliding window of 8 float2 in registers
 //    (the width loop is unrolled by 8, so the rotation is register renaming): one LDS.64 per width step.
 //  * Samples past the row end are staged as -inf: a running sum that has touched one is -inf for every wider
-//    width, so "only widths that fit" (reading A9) needs no masking in the loop.  Widths nmax < w <= 8 ceil(nmax/8)
-//    get a NaN reciprocal: FMNMX drops NaN operands, so they can never win and need no tail loop.
+//    width, so "only widths that fit" (reading A9) needs no masking in the loop.  In the RC = false kernels widths
+//    nmax < w <= 8 ceil(nmax/8) get a NaN reciprocal: FMNMX drops NaN operands, so they can never win.
 //  * arg-max of the general kernel is deferred: the running maximum is advanced with 3-input FMNMX only,
 //    ping-ponging between two register sets so that the value before and after each block of 8 widths are both
 //    live; one compare + one select per block then record the block that last raised it.  After the loop that block
-//    alone is evaluated again from a tile-local prefix sum P kept in shared memory (B_w(t) = P[t+w] - P[t], no
+//    alone is evaluated again from tile-local prefix sums E kept in shared memory (B_w(t) = E[t+w] - E[t], no
 //    dependency chain); the position inside the block rides in the 3 low mantissa bits of the 8 values (a larger tag
 //    is a smaller width), so one maximum gives the width.  Blocks ascend with a strict '>', so exact ties keep the
-//    smallest width (A7).  The SNR written is the running-sum value of the main loop; the re-evaluation only picks
-//    the width and differs from the running sums by fp32 rounding and the 3 tag bits (~1e-6 relative), i.e. only
-//    inside near-ties far below the 1e-3 tie tolerance.
+//    smallest width (A7) for non-negative maxima.  The SNR written is the running-sum value of the main loop; the
+//    re-evaluation only picks the width and differs from the running sums by fp32 rounding and the 3 tag bits (~1e-6
+//    relative), i.e. only inside near-ties far below the 1e-3 tie tolerance.
 //
-// Roofline: 10 B/sample of HBM traffic (4 read + 4 snr + 2 width) against 3*Nmax fp32 lane-ops per sample (add,
-// multiply, compare) at one warp instruction per sub-partition per clock: FP32-issue-bound for Nmax > ~20
-// (DESIGN.md section 7).
+// Roofline: 10 B/sample of HBM traffic (4 read + 4 snr + 2 width) against 2 Nmax FMA-pipe lane-ops per sample
+// (SURVEY.md 8(d)); FP32-issue-bound for Nmax > ~24.
 #include "spd_common.cuh"
+
+#include <mutex>
 
 namespace spd {
 
@@ -44,7 +54,8 @@ constexpr int SW_R       = 8;                        // samples per thread per s
 // 64 threads (tile 1024) for nmax <= SW_SMALL_CTA_NMAX: fewer warps wait on each block barrier; 128 threads (tile 2048)
 // above, where the halo (nmax + 8 positions staged and scanned per tile) would weigh too much on a small tile.
 constexpr int SW_SMALL_CTA_NMAX = 256;
-constexpr int SW_NARROW_NMAX = 24;                   // nmax up to here takes the tagged-maximum kernel (measured crossover on B200: 24..28)
+constexpr int SW_NARROW_NMAX = 32;                   // nmax up to here takes the tagged-maximum kernel (5 tag bits)
+constexpr int SW_NMAX_TAB = 4096 + 16;               // entries of the constant 1/sqrt(w) table (API limit of nmax + padding)
 
 __host__ __device__ inline int zpad(int i) { return i + (i >> 3); }          // one pad float2 per 8: lane stride 72 B
 __host__ __device__ inline int sw_nblk(int nmax) { return (nmax + 7) >> 3; }  // blocks of 8 widths
@@ -53,21 +64,38 @@ __host__ __device__ inline int sw_rt_len(int nmax) { return 8 * sw_nblk(nmax) + 
 
 size_t sweep_table_bytes(int nmax) { return (size_t)sw_rt_len(nmax) * sizeof(float); }
 
+// ---- 1/sqrt(w), w = 1.., as a compile-time table in the constant bank (eq. 4: sigma_N = sqrt(N) sigma) ----
+struct IsqrtTable { float v[SW_NMAX_TAB]; };
+constexpr double sw_csqrt(double x) { double g = x > 1.0 ? x : 1.0; for (int i = 0; i < 64; ++i) g = 0.5 * (g + x / g); return g; }
+constexpr IsqrtTable sw_make_isqrt() { IsqrtTable t{}; for (int i = 0; i < SW_NMAX_TAB; ++i) t.v[i] = (float)(1.0 / sw_csqrt((double)(i + 1))); return t; }
+__constant__ IsqrtTable c_isqrt = sw_make_isqrt();
+
 struct SweepSmem {           // byte offsets into dynamic shared memory (all 16-byte aligned)
-    int z, raw, p2, scan, rtf, total;
+    int z, raw, ea, eb, scan, rtf, total;
     __host__ __device__ SweepSmem(int nmax, int nt)
     {
         const int H = sw_halo(nmax), R = sw_rt_len(nmax), SW_SUB = nt * SW_R, SW_TILE = 2 * SW_SUB;
+        const int groups = (SW_SUB + H) / 8 + 1;                         // groups of 8 prefix sums, 12 floats apart (48 B: conflict-free LDS.128)
         z = 0;                                                           // float2 Z[zpad(SUB + H)]
         raw = z + round_up((zpad(SW_SUB + H) + 1) * 8, 16);              // float raw[TILE + H]
-        p2 = raw + round_up((SW_TILE + H) * 4, 16);                      // float2 P[zpad(SUB + H + 1)]: prefix sums
-        scan = p2 + round_up((zpad(SW_SUB + H + 1) + 1) * 8, 16);        // float2 [2][4]: per-warp totals of the scan (double-buffered by part)
+        ea = raw + round_up((SW_TILE + H) * 4, 16);                      // float EA[groups][12]: exclusive prefix sums of sub-tile A
+        eb = ea + groups * 48;                                           // float EB[groups][12]
+        scan = eb + groups * 48;                                         // float2 [2][4]: per-warp totals of the scan (double-buffered by part)
         rtf = scan + 64;                                                 // float r_w
         total = rtf + round_up(R * 4, 16);
     }
 };
 
 __device__ __forceinline__ float fmax3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }
+
+// (a & mask) | tag in ONE LOP3 (mask must live in a register: with two immediates the compiler emits two instructions)
+__device__ __forceinline__ float tag_bits(float s, int mask, int tag)
+{
+    int d;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(d) : "r"(__float_as_int(s)), "r"(mask), "r"(tag));
+    return __int_as_float(d);
+}
+__device__ __forceinline__ int opaque_reg(int v) { asm volatile("mov.b32 %0, %0;" : "+r"(v)); return v; }
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 {
@@ -105,6 +133,8 @@ cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, f
     return cudaGetLastError();
 }
 
+bool sweep_uses_constant_table(int nmax, int mode) { return mode == SPD_SIGMA_SQRT && (nmax & 7) == 0; }
+
 // Position of a tile in the persistent walk: (row, tile-in-row), advanced by the grid size without 64-bit divisions
 struct TilePos {
     int64_t row; int tr;
@@ -122,10 +152,8 @@ struct TilePos {
 // ---- tile staging -------------------------------------------------------------------------------------------------
 // An interior tile of a 16-byte aligned row is one contiguous run of global memory.  BULK: ONE thread issues a 1-D bulk
 // copy (TMA: cp.async.bulk, completion counted in bytes on an mbarrier) and every thread waits on the barrier's phase;
-// otherwise every thread issues 16-byte cp.async.  Measured on B200 (config-3 shape): the bulk copy is 2.7 % faster for
-// the narrow kernel (Nmax 8, closest to the HBM roofline) and 1.4 % / 6 % SLOWER for the general and the fused kernel,
-// so only the narrow kernel uses it.  Tiles that touch the row end, and rows that are not 16-byte aligned, are staged
-// by all threads (cp.async 16 B where possible, scalar loads otherwise; samples past the row end become -inf).
+// otherwise every thread issues 16-byte cp.async.  Tiles that touch the row end, and rows that are not 16-byte aligned,
+// are staged by all threads (cp.async 16 B where possible, scalar loads otherwise; samples past the row end become -inf).
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
 struct TileStager {
@@ -192,17 +220,48 @@ struct TileStager {
     }
 };
 
+// What every sweep kernel needs from the statistics: y = ((x - mu_hi) - mu_lo) [* 1/sigma when RC]
+struct Norm {
+    float2 mu_hi2, mu_lo2, rs2;
+    __device__ __forceinline__ Norm(const spd_stats_t *st)
+    {
+        const double mu = st->mean;
+        const float mu_hi = (float)mu, mu_lo = (float)(mu - (double)mu_hi), rs = (float)(1.0 / st->sigma);
+        mu_hi2 = make_float2(-mu_hi, -mu_hi); mu_lo2 = make_float2(-mu_lo, -mu_lo); rs2 = make_float2(rs, rs);
+    }
+    template <bool RC>
+    __device__ __forceinline__ float2 apply(float2 v) const
+    {
+        v = __fadd2_rn(__fadd2_rn(v, mu_hi2), mu_lo2);
+        return RC ? __fmul2_rn(v, rs2) : v;
+    }
+};
+
+// 8 groups of one raw tile -> 8 interleaved values (sub-tile A, sub-tile B) of group g
+template <int SW_SUB>
+__device__ __forceinline__ void load_group(const float *raw, int g, float2 (&v)[SW_R])
+{
+    const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
+    const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
+    v[0] = make_float2(a0.x, b0.x); v[1] = make_float2(a0.y, b0.y); v[2] = make_float2(a0.z, b0.z); v[3] = make_float2(a0.w, b0.w);
+    v[4] = make_float2(a1.x, b1.x); v[5] = make_float2(a1.y, b1.y); v[6] = make_float2(a1.z, b1.z); v[7] = make_float2(a1.w, b1.w);
+}
+
 // One block of 8 width steps: advance the 8 packed running sums, scale, fold into the running maxima.
 // out[j] = max(in[j], the 8 SNRs of this block); `in` stays intact so that the caller can tell whether the block
 // raised the maximum.  On entry W[v] = Z[8 tid + a0 + v] (a0 = width offset of the first step); on exit the window
-// has moved by 8.  zp -> Z[8 (tid + kb + 1)] (the next 8 window elements), rp -> r_w of the block (a scalar operand:
-// FMUL2 broadcasts one register to both halves, which costs one register read less than a (r_w, r_w) pair).
+// has moved by 8.  zp -> Z[8 (tid + kb + 1)] (the next 8 window elements).  r_w of the block: RC -> c_isqrt.v[w0 + u]
+// (w0 = 8 kb, warp-uniform: a uniform-register operand of FMUL2); otherwise rp[u] from shared memory (a scalar-broadcast
+// register operand: FMUL2 broadcasts one register to both halves, one register read less than a (r_w, r_w) pair).
+template <bool RC>
 __device__ __forceinline__ void sweep8(float2 (&B)[SW_R], float2 (&W)[SW_R], const float2 (&in)[SW_R], float2 (&out)[SW_R],
-                                       const float2 *__restrict__ zp, const float *__restrict__ rp)
+                                       const float2 *__restrict__ zp, const float *__restrict__ rp, int w0)
 {
 #pragma unroll
     for (int u = 0; u < 8; u += 2) {
-        const float2 rr = *reinterpret_cast<const float2 *>(rp + u);              // r_w of the two widths: scalar-broadcast operands of FMUL2
+        float2 rr;
+        if (RC) rr = make_float2(c_isqrt.v[w0 + u], c_isqrt.v[w0 + u + 1]);
+        else rr = *reinterpret_cast<const float2 *>(rp + u);
         const float2 r0 = make_float2(rr.x, rr.x), r1 = make_float2(rr.y, rr.y);
         const float2 n0 = zp[u], n1 = zp[u + 1];
 #pragma unroll
@@ -220,14 +279,14 @@ __device__ __forceinline__ void sweep8(float2 (&B)[SW_R], float2 (&W)[SW_R], con
     }
 }
 
-// record, per running sum, whether the block of widths that just ended raised the maximum
-__device__ __forceinline__ void note_block(const float2 (&now)[SW_R], const float2 (&old)[SW_R], int w0,
-                                           int (&w0x)[SW_R], int (&w0y)[SW_R])
+// record, per running sum, whether the block of widths that just ended raised the maximum (kb = index of the block)
+__device__ __forceinline__ void note_block(const float2 (&now)[SW_R], const float2 (&old)[SW_R], int kb,
+                                           int (&kx)[SW_R], int (&ky)[SW_R])
 {
 #pragma unroll
     for (int j = 0; j < SW_R; ++j) {
-        w0x[j] = (now[j].x > old[j].x) ? w0 : w0x[j];
-        w0y[j] = (now[j].y > old[j].y) ? w0 : w0y[j];
+        kx[j] = (now[j].x > old[j].x) ? kb : kx[j];
+        ky[j] = (now[j].y > old[j].y) ? kb : ky[j];
     }
 }
 
@@ -271,7 +330,32 @@ __device__ __forceinline__ void store_planes(float *__restrict__ snr, uint16_t *
     }
 }
 
-template <int SW_THREADS>
+// Width inside the winning block of ONE sample (position J of the thread's 8, J a compile-time constant), from the
+// exclusive prefix sums E of its sub-tile: B_w(t) = E[t + w] - E[t].  E is kept in groups of 8 (12 floats apart), group
+// G = tid + kb holds E[8 tid + 8 kb ..+7], so the 8 candidates E[t + 8 kb + 1 .. + 8] are elements J+1..7 of group G
+// and 0..J of group G + 1: at most four 16-byte loads, no address arithmetic per candidate.  The position inside the
+// block rides in the 3 low mantissa bits (7 - g: exact ties keep the smallest width); a tagged -inf or NaN (width
+// past the row end / past nmax) is a NaN, which FMNMX drops.
+template <int J>
+__device__ __forceinline__ int width_in_block(const float *__restrict__ E, const float *__restrict__ rtf, int tid, int kb, float p0, int mask)
+{
+    const float4 *eg = reinterpret_cast<const float4 *>(E + (tid + kb) * 12);       // group G; G + 1 is 3 float4 further
+    float e[16];
+    if (J + 1 < 4) { const float4 q = eg[0]; e[0] = q.x; e[1] = q.y; e[2] = q.z; e[3] = q.w; }
+    if (J + 1 < 8) { const float4 q = eg[1]; e[4] = q.x; e[5] = q.y; e[6] = q.z; e[7] = q.w; }
+    { const float4 q = eg[3]; e[8] = q.x; e[9] = q.y; e[10] = q.z; e[11] = q.w; }
+    if (J >= 4) { const float4 q = eg[4]; e[12] = q.x; e[13] = q.y; e[14] = q.z; e[15] = q.w; }
+    const float4 *rq = reinterpret_cast<const float4 *>(rtf + 8 * kb);
+    const float4 ra = rq[0], rb = rq[1];
+    const float r[8] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y, rb.z, rb.w};
+    float s[8];
+#pragma unroll
+    for (int g = 0; g < 8; ++g) s[g] = tag_bits((e[J + 1 + g] - p0) * r[g], mask, 7 - g);
+    const float m = fmaxf(fmax3(fmax3(s[0], s[1], s[2]), s[3], s[4]), fmax3(s[5], s[6], s[7]));
+    return 8 * kb + 8 - (__float_as_int(m) & 7);
+}
+
+template <int SW_THREADS, bool RC>
 __global__ void __launch_bounds__(SW_THREADS, 512 / SW_THREADS)
 boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                  const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
@@ -282,23 +366,23 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
     const SweepSmem lay(nmax, SW_THREADS);
     float2 *Z   = reinterpret_cast<float2 *>(smem_raw + lay.z);
     float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
-    float2 *P2  = reinterpret_cast<float2 *>(smem_raw + lay.p2);      // prefix sums of y: (sub-tile A, sub-tile B), zpad layout
+    float  *EA  = reinterpret_cast<float *>(smem_raw + lay.ea);       // exclusive prefix sums of y, sub-tile A, groups of 8 at 12-float pitch
+    float  *EB  = reinterpret_cast<float *>(smem_raw + lay.eb);
     float2 *scan = reinterpret_cast<float2 *>(smem_raw + lay.scan);   // [2][4] per-warp totals of the tile prefix scan
-    float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);      // r_w = 1 / sigma_w
+    float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);      // r_w (the width search reads it with a per-lane index)
 
     const int tid = threadIdx.x;
     const int lane = tid & 31, wid = tid >> 5;
     const int nblk = sw_nblk(nmax);
     const int H = sw_halo(nmax);
-    const int LRAW = SW_TILE + H;                 // raw floats per tile: x[T0 .. T0 + 2048 + H)
+    const int LRAW = SW_TILE + H;                 // raw floats per tile: x[T0 .. T0 + TILE + H)
     const int LZ = SW_SUB + H;                    // interleaved positions (a multiple of 8)
     const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
-    const double mu = st->mean;
-    const float mu_hi = (float)mu, mu_lo = (float)(mu - (double)mu_hi);
-    const float2 mu_hi2 = make_float2(-mu_hi, -mu_hi), mu_lo2 = make_float2(-mu_lo, -mu_lo);
+    const Norm norm(st);
     const float NINF = __int_as_float(0xff800000);
+    const int mask7 = opaque_reg(~7);
 
-    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
+    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = RC ? c_isqrt.v[w] : __ldg(table + w);
 
     int64_t tile = blockIdx.x;
     TilePos pos(blockIdx.x, tiles_per_row);
@@ -312,22 +396,21 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
         const int64_t T0 = (int64_t)pos.tr * SW_TILE;
         pos = pos.next(gridDim.x, tiles_per_row);                                  // the tile after this one
         stg.wait();
-        __syncthreads();                           // raw tile landed; everyone is done with the previous Z / P
+        __syncthreads();                           // raw tile landed; everyone is done with the previous Z / E
 
         // ---- per-thread state ---------------------------------------------------------------------------------------
         float2 B[SW_R], W[SW_R], bestA[SW_R], bestB[SW_R];
-        int w0x[SW_R], w0y[SW_R];
+        int kx[SW_R], ky[SW_R];
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) {
             B[j] = make_float2(0.f, 0.f);
             bestA[j] = make_float2(NINF, NINF);
-            w0x[j] = 0; w0y[j] = 0;
+            kx[j] = 0; ky[j] = 0;
         }
 
         // ---- staging, one pass: every thread takes groups of 8 consecutive positions (part 0: its own 8 samples, whose
-        //      y values stay in registers as the first window), forms y = x - mu (two-term fp32 subtract), writes the
-        //      interleaved Z and the tile-local inclusive prefix sums P[i + 1] = y[0] + ... + y[i] of both sub-tiles
-        //      (only the width search reads P)
+        //      y values stay in registers as the first window), forms y, writes the interleaved Z and the tile-local
+        //      EXCLUSIVE prefix sums E[i] = y[0] + ... + y[i-1] of both sub-tiles (only the width search reads E)
         {
             float2 carry = make_float2(0.f, 0.f);
             for (int part = 0; part < nparts; ++part) {
@@ -339,13 +422,10 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
                 float2 *tot = scan + 4 * (part & 1);
                 if (wact) {
                     if (act) {
-                        const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
-                        const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
-                        v[0] = make_float2(a0.x, b0.x); v[1] = make_float2(a0.y, b0.y); v[2] = make_float2(a0.z, b0.z); v[3] = make_float2(a0.w, b0.w);
-                        v[4] = make_float2(a1.x, b1.x); v[5] = make_float2(a1.y, b1.y); v[6] = make_float2(a1.z, b1.z); v[7] = make_float2(a1.w, b1.w);
+                        load_group<SW_SUB>(raw, g, v);
 #pragma unroll
                         for (int j = 0; j < SW_R; ++j) {
-                            v[j] = __fadd2_rn(__fadd2_rn(v[j], mu_hi2), mu_lo2);
+                            v[j] = norm.apply<RC>(v[j]);
                             Z[9 * g + j] = v[j];                 // zpad(8 g + j) = 9 g + j
                         }
                     } else {
@@ -378,12 +458,16 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
                     if (w < wid) off = __fadd2_rn(off, t);
                     carry = __fadd2_rn(carry, t);
                 }
-                if (act) {
+                if (act) {                                       // group g of E: off, off + v0, ..., off + v6 (v is the inclusive scan)
+                    float2 e[SW_R];
+                    e[0] = off;
 #pragma unroll
-                    for (int j = 0; j < SW_R; ++j) P2[zpad(8 * g + j + 1)] = __fadd2_rn(v[j], off);
+                    for (int j = 1; j < SW_R; ++j) e[j] = __fadd2_rn(v[j - 1], off);
+                    float4 *da = reinterpret_cast<float4 *>(EA + 12 * g), *db = reinterpret_cast<float4 *>(EB + 12 * g);
+                    da[0] = make_float4(e[0].x, e[1].x, e[2].x, e[3].x); da[1] = make_float4(e[4].x, e[5].x, e[6].x, e[7].x);
+                    db[0] = make_float4(e[0].y, e[1].y, e[2].y, e[3].y); db[1] = make_float4(e[4].y, e[5].y, e[6].y, e[7].y);
                 }
             }
-            if (tid == 0) P2[0] = make_float2(0.f, 0.f);
         }
 
         // ---- main loop: blocks of 8 widths, the running maximum ping-pongs between bestA and bestB ---------------------
@@ -391,51 +475,43 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
             const float2 *zp = Z + 9 * (tid + 1);                // zpad(8 tid + 8 kb + 8 + u) = 9 (tid + kb + 1) + u
             const float *rp = rtf;
             int kb = 0;
-            for (; kb + 2 <= nblk; kb += 2) {
-                sweep8(B, W, bestA, bestB, zp, rp);
-                note_block(bestB, bestA, 8 * kb, w0x, w0y);
-                sweep8(B, W, bestB, bestA, zp + 9, rp + 8);
-                note_block(bestA, bestB, 8 * kb + 8, w0x, w0y);
+            int kbv = opaque_reg(0);      // the block index as a per-thread value for note_block: the loop counter itself stays
+                                          // warp-uniform, so c_isqrt.v[8 kb + u] is loaded into a uniform register (LDCU)
+            for (; kb + 2 <= nblk; kb += 2, kbv += 2) {
+                sweep8<RC>(B, W, bestA, bestB, zp, rp, 8 * kb);
+                note_block(bestB, bestA, kbv, kx, ky);
+                sweep8<RC>(B, W, bestB, bestA, zp + 9, rp + 8, 8 * kb + 8);
+                note_block(bestA, bestB, kbv + 1, kx, ky);
                 zp += 18; rp += 16;
             }
             if (kb < nblk) {
-                sweep8(B, W, bestA, bestB, zp, rp);
-                note_block(bestB, bestA, 8 * kb, w0x, w0y);
+                sweep8<RC>(B, W, bestA, bestB, zp, rp, 8 * kb);
+                note_block(bestB, bestA, kbv, kx, ky);
 #pragma unroll
                 for (int j = 0; j < SW_R; ++j) bestA[j] = bestB[j];
             }
         }
         float2 (&best)[SW_R] = bestA;
-        __syncthreads();                           // P (written before the main loop) is complete for every warp
+        __syncthreads();                           // E (written before the main loop) is complete for every warp
 
-        // ---- width search inside the winning block, from the prefix sums: B_w(t) = P[t + w] - P[t] ------------------
+        // ---- width search inside the winning block -----------------------------------------------------------------
         int wx[SW_R], wy[SW_R];
-#pragma unroll
-        for (int j = 0; j < SW_R; ++j) {
-            const float2 p0 = P2[9 * tid + j];                                    // P[t], t = 8 tid + j
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int w0 = h ? w0y[j] : w0x[j];
-                const float p0h = h ? p0.y : p0.x;
-                const float *pe = reinterpret_cast<const float *>(P2 + 9 * (tid + (w0 >> 3))) + h;   // zpad(8 tid + w0 + c) = 9 (tid + w0/8) + c + (c >> 3)
-                const float4 *rq = reinterpret_cast<const float4 *>(rtf + w0);
-                const float4 ra = rq[0], rb = rq[1];
-                const float r[8] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y, rb.z, rb.w};
-                float s[8];
-#pragma unroll
-                for (int g = 0; g < 8; ++g) { const int c = j + g + 1; s[g] = (pe[2 * (c + (c >> 3))] - p0h) * r[g]; }
-                // the position inside the block rides in the 3 low mantissa bits (7 - g: ties keep the smallest width);
-                // a tagged -inf or NaN (width past the row end / past nmax) is a NaN, which FMNMX drops
-#pragma unroll
-                for (int g = 0; g < 8; ++g) s[g] = __int_as_float((__float_as_int(s[g]) & ~7) | (7 - g));
-                const float m = fmaxf(fmax3(fmax3(s[0], s[1], s[2]), s[3], s[4]), fmax3(s[5], s[6], s[7]));
-                const int w = 7 - (__float_as_int(m) & 7);
-                if (h) wy[j] = w0 + w + 1; else wx[j] = w0 + w + 1;
-            }
+        if (width) {
+            const float4 *oa = reinterpret_cast<const float4 *>(EA + 12 * tid), *ob = reinterpret_cast<const float4 *>(EB + 12 * tid);
+            const float4 a0 = oa[0], a1 = oa[1], b0 = ob[0], b1 = ob[1];          // E[t] of the thread's own 8 + 8 samples
+            const float pa[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w}, pb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+            wx[0] = width_in_block<0>(EA, rtf, tid, kx[0], pa[0], mask7); wy[0] = width_in_block<0>(EB, rtf, tid, ky[0], pb[0], mask7);
+            wx[1] = width_in_block<1>(EA, rtf, tid, kx[1], pa[1], mask7); wy[1] = width_in_block<1>(EB, rtf, tid, ky[1], pb[1], mask7);
+            wx[2] = width_in_block<2>(EA, rtf, tid, kx[2], pa[2], mask7); wy[2] = width_in_block<2>(EB, rtf, tid, ky[2], pb[2], mask7);
+            wx[3] = width_in_block<3>(EA, rtf, tid, kx[3], pa[3], mask7); wy[3] = width_in_block<3>(EB, rtf, tid, ky[3], pb[3], mask7);
+            wx[4] = width_in_block<4>(EA, rtf, tid, kx[4], pa[4], mask7); wy[4] = width_in_block<4>(EB, rtf, tid, ky[4], pb[4], mask7);
+            wx[5] = width_in_block<5>(EA, rtf, tid, kx[5], pa[5], mask7); wy[5] = width_in_block<5>(EB, rtf, tid, ky[5], pb[5], mask7);
+            wx[6] = width_in_block<6>(EA, rtf, tid, kx[6], pa[6], mask7); wy[6] = width_in_block<6>(EB, rtf, tid, ky[6], pb[6], mask7);
+            wx[7] = width_in_block<7>(EA, rtf, tid, kx[7], pa[7], mask7); wy[7] = width_in_block<7>(EB, rtf, tid, ky[7], pb[7], mask7);
         }
 
         // a NaN reciprocal table (LINEAR mode fed stats of another Nmax) must surface: fmaxf drops NaN operands
-        if (rtf[0] != rtf[0]) {
+        if (!RC && rtf[0] != rtf[0]) {
 #pragma unroll
             for (int j = 0; j < SW_R; ++j) best[j] = make_float2(rtf[0], rtf[0]);
         }
@@ -473,7 +549,7 @@ __device__ __noinline__ int replay_width(const float *__restrict__ zh, int pos, 
     return nmax;                                   // not reached for finite input
 }
 
-template <int SW_THREADS>
+template <int SW_THREADS, bool RC>
 __global__ void __launch_bounds__(SW_THREADS, 512 / SW_THREADS)
 boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                     const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
@@ -492,12 +568,13 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
     const int H = sw_halo(nmax);
     const int LRAW = SW_TILE + H, LZ = SW_SUB + H;
     const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
-    const double mu = st->mean;
-    const float mu_hi = (float)mu, mu_lo = (float)(mu - (double)mu_hi);
-    const float2 mu_hi2 = make_float2(-mu_hi, -mu_hi), mu_lo2 = make_float2(-mu_lo, -mu_lo);
+    const Norm norm(st);
     const float NINF = __int_as_float(0xff800000);
 
-    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
+    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = RC ? c_isqrt.v[w] : __ldg(table + w);
+    // a NaN reciprocal table (LINEAR mode fed stats of another Nmax): NaN >= threshold is false everywhere, which would
+    // read as "no detections"; report the misuse as count = ~0 instead (spd.h)
+    if (!RC && blockIdx.x == 0 && tid == 0) { const float r0 = __ldg(table); if (r0 != r0) *count = ~0ULL; }
 
     int64_t tile = blockIdx.x;
     TilePos pos(blockIdx.x, tiles_per_row);
@@ -517,13 +594,11 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
         for (int part = 0; part < nparts; ++part) {
             const int g = part * SW_THREADS + tid;
             if (8 * g < LZ) {
-                const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
-                const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
-                float2 v[SW_R] = {make_float2(a0.x, b0.x), make_float2(a0.y, b0.y), make_float2(a0.z, b0.z), make_float2(a0.w, b0.w),
-                                  make_float2(a1.x, b1.x), make_float2(a1.y, b1.y), make_float2(a1.z, b1.z), make_float2(a1.w, b1.w)};
+                float2 v[SW_R];
+                load_group<SW_SUB>(raw, g, v);
 #pragma unroll
                 for (int j = 0; j < SW_R; ++j) {
-                    v[j] = __fadd2_rn(__fadd2_rn(v[j], mu_hi2), mu_lo2);
+                    v[j] = norm.apply<RC>(v[j]);
                     Z[9 * g + j] = v[j];
                     if (part == 0) W[j] = v[j];
                 }
@@ -537,7 +612,7 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
         {
             const float2 *zp = Z + 9 * (tid + 1);
             const float *rp = rtf;
-            for (int kb = 0; kb < nblk; ++kb, zp += 9, rp += 8) sweep8(B, W, best, best, zp, rp);
+            for (int kb = 0; kb < nblk; ++kb, zp += 9, rp += 8) sweep8<RC>(B, W, best, best, zp, rp, 8 * kb);
         }
 
         // ---- threshold; hits replay their own running sums to get the width ------------------------------------------
@@ -564,22 +639,24 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Narrow searches (nmax <= SW_NARROW_NMAX; the tag has room for 32 widths): the fixed per-sample cost of the general kernel (prefix scan + width search, about 100
-// clocks per 32 samples) is larger than the width loop itself, so here the arg-max rides along with the maximum:
-// beside the exact running maximum a second one is kept over TAGGED values, (bits(s) & ~31) | (32 - w).  A larger
-// tag is a smaller width, so exact ties keep the smallest width (A7); values closer than 32 ulp (4e-6 relative, far
-// inside the 1e-3 tie tolerance of DESIGN.md section 5) may resolve either way.  The SNR written is the exact maximum.
-// A tagged -inf (a window past the row end) is a NaN, which FMNMX drops.  No scan, no width search, no bookkeeping.
-template <int KB>
+// Narrow searches (nmax <= SW_NARROW_NMAX = 32, the room of a 5-bit tag): the fixed per-sample cost of the general
+// kernel (prefix scan + width search) is larger than the width loop itself, so here the arg-max rides along with the
+// maximum: beside the exact running maximum a second one is kept over TAGGED values, (bits(s) & ~31) | (32 - w), one
+// LOP3 per value.  A larger tag is a smaller width, so exact ties keep the smallest width (A7) for non-negative maxima;
+// values closer than 32 ulp (4e-6 relative, far inside the 1e-3 tie tolerance of DESIGN.md section 5) may resolve
+// either way.  The SNR written is the exact maximum.  A tagged -inf (a window past the row end) or NaN (a width past
+// nmax) is a NaN, which FMNMX drops.  No scan, no width search, no bookkeeping.
+template <int KB, bool RC>
 __device__ __forceinline__ void sweep8_tagged(float2 (&B)[SW_R], float2 (&W)[SW_R], float2 (&best)[SW_R], float2 (&tbest)[SW_R],
-                                              const float2 *__restrict__ zp, const float *__restrict__ rp)
+                                              const float2 *__restrict__ zp, const float *__restrict__ rp, int mask)
 {
 #pragma unroll
     for (int u = 0; u < 8; u += 2) {
-        const float2 rr = *reinterpret_cast<const float2 *>(rp + u);
+        float2 rr;
+        if (RC) rr = make_float2(c_isqrt.v[8 * KB + u], c_isqrt.v[8 * KB + u + 1]);
+        else rr = *reinterpret_cast<const float2 *>(rp + u);
         const float2 r0 = make_float2(rr.x, rr.x), r1 = make_float2(rr.y, rr.y);
         const float2 n0 = zp[u], n1 = zp[u + 1];
-        constexpr int MASK = ~31;
         const int c0 = 32 - (8 * KB + u + 1), c1 = c0 - 1;              // 32 - w for the two widths of this step
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) {
@@ -589,15 +666,15 @@ __device__ __forceinline__ void sweep8_tagged(float2 (&B)[SW_R], float2 (&W)[SW_
             const float2 s1 = __fmul2_rn(B[j], r1);
             best[j].x = fmax3(best[j].x, s0.x, s1.x);
             best[j].y = fmax3(best[j].y, s0.y, s1.y);
-            tbest[j].x = fmax3(tbest[j].x, __int_as_float((__float_as_int(s0.x) & MASK) | c0), __int_as_float((__float_as_int(s1.x) & MASK) | c1));
-            tbest[j].y = fmax3(tbest[j].y, __int_as_float((__float_as_int(s0.y) & MASK) | c0), __int_as_float((__float_as_int(s1.y) & MASK) | c1));
+            tbest[j].x = fmax3(tbest[j].x, tag_bits(s0.x, mask, c0), tag_bits(s1.x, mask, c1));
+            tbest[j].y = fmax3(tbest[j].y, tag_bits(s0.y, mask, c0), tag_bits(s1.y, mask, c1));
         }
         W[u] = n0;
         W[u + 1] = n1;
     }
 }
 
-template <int SW_THREADS>
+template <int SW_THREADS, bool RC>
 __global__ void __launch_bounds__(SW_THREADS, 640 / SW_THREADS)
 boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                         const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
@@ -615,12 +692,11 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
     const int H = sw_halo(nmax);
     const int LRAW = SW_TILE + H, LZ = SW_SUB + H;
     const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
-    const double mu = st->mean;
-    const float mu_hi = (float)mu, mu_lo = (float)(mu - (double)mu_hi);
-    const float2 mu_hi2 = make_float2(-mu_hi, -mu_hi), mu_lo2 = make_float2(-mu_lo, -mu_lo);
+    const Norm norm(st);
     const float NINF = __int_as_float(0xff800000);
+    const int mask31 = opaque_reg(~31);
 
-    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
+    if (!RC) for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
 
     int64_t tile = blockIdx.x;
     TilePos pos(blockIdx.x, tiles_per_row);
@@ -640,13 +716,11 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
         for (int part = 0; part < nparts; ++part) {
             const int g = part * SW_THREADS + tid;
             if (8 * g < LZ) {
-                const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
-                const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
-                float2 v[SW_R] = {make_float2(a0.x, b0.x), make_float2(a0.y, b0.y), make_float2(a0.z, b0.z), make_float2(a0.w, b0.w),
-                                  make_float2(a1.x, b1.x), make_float2(a1.y, b1.y), make_float2(a1.z, b1.z), make_float2(a1.w, b1.w)};
+                float2 v[SW_R];
+                load_group<SW_SUB>(raw, g, v);
 #pragma unroll
                 for (int j = 0; j < SW_R; ++j) {
-                    v[j] = __fadd2_rn(__fadd2_rn(v[j], mu_hi2), mu_lo2);
+                    v[j] = norm.apply<RC>(v[j]);
                     Z[9 * g + j] = v[j];
                     if (part == 0) W[j] = v[j];
                 }
@@ -658,15 +732,15 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); tbest[j] = make_float2(NINF, NINF); }
         const float2 *zp = Z + 9 * (tid + 1);
-        sweep8_tagged<0>(B, W, best, tbest, zp, rtf);
-        if (nblk > 1) sweep8_tagged<1>(B, W, best, tbest, zp + 9, rtf + 8);
-        if (nblk > 2) sweep8_tagged<2>(B, W, best, tbest, zp + 18, rtf + 16);
-        if (nblk > 3) sweep8_tagged<3>(B, W, best, tbest, zp + 27, rtf + 24);
+        sweep8_tagged<0, RC>(B, W, best, tbest, zp, rtf, mask31);
+        if (nblk > 1) sweep8_tagged<1, RC>(B, W, best, tbest, zp + 9, rtf + 8, mask31);
+        if (nblk > 2) sweep8_tagged<2, RC>(B, W, best, tbest, zp + 18, rtf + 16, mask31);
+        if (nblk > 3) sweep8_tagged<3, RC>(B, W, best, tbest, zp + 27, rtf + 24, mask31);
 
         int wx[SW_R], wy[SW_R];
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) { wx[j] = 32 - (__float_as_int(tbest[j].x) & 31); wy[j] = 32 - (__float_as_int(tbest[j].y) & 31); }
-        if (rtf[0] != rtf[0]) {                     // NaN table (LINEAR mode fed stats of another Nmax) must surface
+        if (!RC && rtf[0] != rtf[0]) {              // NaN table (LINEAR mode fed stats of another Nmax) must surface
 #pragma unroll
             for (int j = 0; j < SW_R; ++j) { best[j] = make_float2(rtf[0], rtf[0]); wx[j] = 1; wy[j] = 1; }
         }
@@ -675,22 +749,55 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
     cp_async_commit_wait_all();
 }
 
+// ---- launch: one resident wave of persistent CTAs.  The occupancy of a (kernel, shared-memory size, device) is looked up
+// once and cached, and the kernel's dynamic shared-memory limit is only ever raised (the queries cost ~40 us per launch
+// otherwise; config 1 is launch-latency-bound).
+struct GridCache {
+    std::mutex mu;
+    struct Entry { const void *fn; int smem, dev, ctas; };
+    Entry e[256];
+    int n = 0;
+    int limit(const void *fn, int dev) const          // largest dynamic shared-memory size set for this kernel so far
+    {
+        int m = 0;
+        for (int i = 0; i < n; ++i) if (e[i].fn == fn && e[i].dev == dev && e[i].smem > m) m = e[i].smem;
+        return m;
+    }
+};
+static GridCache g_grid_cache;
+
 template <typename K>
 static cudaError_t persistent_grid(K kernel, int threads, int smem, int64_t tiles, unsigned *grid)
 {
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    int dev = 0, sms = 0, per_sm = 0;
-    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem)) != cudaSuccess) return e;
-    if (per_sm < 1) return cudaErrorInvalidConfiguration;
-    const int64_t wave = (int64_t)sms * per_sm;                 // persistent: one resident wave walks all tiles
-    *grid = (unsigned)(tiles < wave ? tiles : wave);
+    const void *fn = reinterpret_cast<const void *>(kernel);
+    int wave = 0;
+    {
+        std::lock_guard<std::mutex> lk(g_grid_cache.mu);
+        for (int i = 0; i < g_grid_cache.n; ++i) {
+            const GridCache::Entry &c = g_grid_cache.e[i];
+            if (c.fn == fn && c.smem == smem && c.dev == dev) { wave = c.ctas; break; }
+        }
+        if (wave == 0) {
+            int sms = 0, per_sm = 0;
+            const bool full = g_grid_cache.n >= 256;             // table full: set the attribute every time, never below a cached size
+            const int lim = g_grid_cache.limit(fn, dev);
+            if (full || smem > lim)
+                if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem > lim ? smem : lim)) != cudaSuccess) return e;
+            if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+            if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem)) != cudaSuccess) return e;
+            if (per_sm < 1) return cudaErrorInvalidConfiguration;
+            wave = sms * per_sm;                                 // persistent: one resident wave walks all tiles
+            if (!full) g_grid_cache.e[g_grid_cache.n++] = GridCache::Entry{fn, smem, dev, wave};
+        }
+    }
+    *grid = (unsigned)(tiles < wave ? tiles : (int64_t)wave);
     return cudaSuccess;
 }
 
-template <int NT>
+template <int NT, bool RC>
 static cudaError_t launch_sweep_nt(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
                                    const float *d_table, int nmax, float *snr, uint16_t *width,
                                    bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
@@ -703,29 +810,33 @@ static cudaError_t launch_sweep_nt(const float *x, int64_t n_dm, int64_t n_t, in
     cudaError_t e;
     if (fused) {
         const FusedSmem lay(nmax, NT);
-        if ((e = persistent_grid(boxcar_search_fused<NT>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_search_fused<NT><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax,
-                                                            threshold, out, capacity, d_count);
+        if ((e = persistent_grid(boxcar_search_fused<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_search_fused<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax,
+                                                                threshold, out, capacity, d_count);
     } else if (nmax <= SW_NARROW_NMAX) {
         const FusedSmem lay(nmax, NT);
-        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep_narrow<NT><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
+        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep_narrow<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
     } else {
         const SweepSmem lay(nmax, NT);
-        if ((e = persistent_grid(boxcar_snr_sweep<NT>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep<NT><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
+        if ((e = persistent_grid(boxcar_snr_sweep<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
     }
     return cudaGetLastError();
 }
 
+// rc = sweep_uses_constant_table(nmax, mode): eq. 4 with nmax a multiple of 8 (d_table is then not read)
 cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
-                         const float *d_table, int nmax, float *snr, uint16_t *width,
+                         const float *d_table, int nmax, bool rc, float *snr, uint16_t *width,
                          bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
                          unsigned long long *d_count, cudaStream_t s)
 {
-    if (nmax <= SW_SMALL_CTA_NMAX)
-        return launch_sweep_nt<64>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
-    return launch_sweep_nt<128>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
+    if (nmax <= SW_SMALL_CTA_NMAX) {
+        if (rc) return launch_sweep_nt<64, true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
+        return launch_sweep_nt<64, false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
+    }
+    if (rc) return launch_sweep_nt<128, true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
+    return launch_sweep_nt<128, false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
 }
 
 }  // namespace spd

@@ -193,8 +193,8 @@ def test_sweep_linear_with_wrong_nmax_is_all_nan(P):
         g_snr, _, (d, _, _) = gpu_sweep(x, st, nmax, "linear")
         assert np.all(np.isnan(g_snr))
         from gpu_util import gpu_fused
-        rec, total = gpu_fused(d, st, nmax, "linear", 3.0)    # NaN >= threshold is false: the fused search reports nothing
-        assert total == 0
+        with pytest.raises(P.SpdError):                   # the fused search reports the misuse as count = 2^64 - 1 (spd.h)
+            gpu_fused(d, st, nmax, "linear", 3.0)
 
 
 def test_sweep_without_width_plane(P):
