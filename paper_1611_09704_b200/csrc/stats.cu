@@ -1,15 +1,22 @@
-// stats.cu -- step 1 of the path: mean and standard deviation (section 2.1).
+// stats.cu -- step 1 of the path: mean and standard deviation (section 2.1), and the "true"
+// sigma_Nmax of eq. 5 (section 2.2) IN THE SAME PASS over x.
 //
-// Kernel 1 (stats_partial): the array is cut into equal chunks of 4096 samples; every thread runs the
-// streaming update eq. 1 over a fixed run of 16 samples (division-free: 1/(j(j-1)) are compile-time
-// constants), the 32 runs of a warp are merged pairwise with eq. 2 through shuffles, and the warp's
-// 512-sample partial is merged (eq. 2, fp64) into a per-warp accumulator.  Each CTA writes one
-// (m, T, S) partial.  Kernel 2 (stats_finalize) merges the partials with eq. 2 in index order (fp64,
-// fixed order => bit-reproducible) and writes mu = T/n, sigma = sqrt(S/n).
+// Kernel 1: the array is cut into equal chunks of 4096 samples; every thread runs the streaming update eq. 1 over a
+// fixed run of 16 samples (division-free: 1/(j(j-1)) are compile-time constants), the 32 runs of a warp are merged
+// pairwise with eq. 2 through shuffles, and the warp's 512-sample partial is merged (eq. 2, fp64) into a per-warp
+// accumulator.  Each CTA writes one (m, T, S) partial.  Two variants:
+//   stats_partial      (nmax_for_sigma = 0): 16-byte streaming loads straight into registers.
+//   stats_partial_win  (nmax_for_sigma > 0): the chunk and its nmax-1 halo samples are staged in shared memory ONCE;
+//                      the same data gives the sample statistics and the Nmax-sample boxcar SUMS of every full window
+//                      (first window of a thread from a tile-local fp32 prefix scan, the next 15 slide), which go
+//                      through the same eq. 1 / eq. 2 reduction.  x is read once (plus the halo, which hits L2).
+// Kernel 2 (stats_finalize) merges the partials with eq. 2 in index order (fp64, fixed order => bit-reproducible) and
+// writes mu = T/n, sigma = sqrt(S/n), sigma_nmax.
 //
-// Precision (reading A4): fp32 inside a warp-chunk (<= 512 samples), fp64 above it.  All
-// samples are shifted by K = x[0][0] before they enter eq. 1 (eq. 1/2 are applied to x - K; S is
-// shift-invariant and T is un-shifted at the end), which keeps fp32 accurate when |mu| >> sigma.
+// Precision (reading A4): fp32 inside a warp-chunk (<= 512 values), fp64 above it.  All samples are shifted
+// by a per-CTA constant K before they enter eq. 1 (eq. 1/2 are applied to x - K; S is shift-invariant and T is
+// un-shifted in fp64 when the CTA writes its partial), which keeps fp32 accurate when |mu| >> sigma.  K is the MEAN of
+// the first chunk the CTA works on, so one outlier sample cannot spoil it.
 //
 // Roofline: pure HBM stream, 4 B/sample read.
 #include "spd_common.cuh"
@@ -39,6 +46,16 @@ __device__ __forceinline__ void chan_push(float &T, float &S, float x)
     S = fmaf(d * d, 1.0f / (float)(J * (J - 1)), S);
 }
 
+// eq. 1 over a full run of 16 values
+__device__ __forceinline__ void chan_run16(const float (&v)[ST_RUN], float &T, float &S)
+{
+    T = v[0]; S = 0.0f;
+    chan_push<2>(T, S, v[1]);   chan_push<3>(T, S, v[2]);   chan_push<4>(T, S, v[3]);   chan_push<5>(T, S, v[4]);
+    chan_push<6>(T, S, v[5]);   chan_push<7>(T, S, v[6]);   chan_push<8>(T, S, v[7]);   chan_push<9>(T, S, v[8]);
+    chan_push<10>(T, S, v[9]);  chan_push<11>(T, S, v[10]); chan_push<12>(T, S, v[11]); chan_push<13>(T, S, v[12]);
+    chan_push<14>(T, S, v[13]); chan_push<15>(T, S, v[14]); chan_push<16>(T, S, v[15]);
+}
+
 // eq. 2 for two partials of EQUAL size m: S = S1 + S2 + (T1 - T2)^2 / (2m)
 __device__ __forceinline__ void merge_equal(float &T, float &S, float T2, float S2, float inv_2m)
 {
@@ -47,166 +64,291 @@ __device__ __forceinline__ void merge_equal(float &T, float &S, float T2, float 
     T += T2;
 }
 
+// the 32 full runs of a warp -> one 512-value partial on every lane (eq. 2, equal sizes at each level)
+__device__ __forceinline__ void warp_merge_full(float &T, float &S)
+{
+#pragma unroll
+    for (int lvl = 0; lvl < 5; ++lvl) {
+        float T2 = __shfl_xor_sync(0xffffffffu, T, 1 << lvl);
+        float S2 = __shfl_xor_sync(0xffffffffu, S, 1 << lvl);
+        merge_equal(T, S, T2, S2, 1.0f / (float)(2 * (ST_RUN << lvl)));
+    }
+}
+
+// runs of any length (ragged chunk): eq. 2 in fp64, the left operand always being the lower lanes
+__device__ __forceinline__ void warp_merge_ragged(Tri &t, int lane)
+{
+#pragma unroll
+    for (int lvl = 0; lvl < 5; ++lvl) {
+        Tri o;
+        o.m = __shfl_xor_sync(0xffffffffu, t.m, 1 << lvl);
+        o.T = __shfl_xor_sync(0xffffffffu, t.T, 1 << lvl);
+        o.S = __shfl_xor_sync(0xffffffffu, t.S, 1 << lvl);
+        if ((lane >> lvl) & 1) { Tri a = o; tri_merge(a, t); t = a; } else tri_merge(t, o);
+    }
+}
+
+// eq. 1 with a run-time j over the first `cnt` of up to 16 values (ragged run)
+__device__ __forceinline__ Tri chan_run_ragged(const float (&v)[ST_RUN], int cnt)
+{
+    float T = 0.0f, S = 0.0f;
+    for (int k = 0; k < ST_RUN; ++k) {
+        if (k < cnt) {
+            if (k == 0) { T = v[0]; S = 0.0f; }
+            else { T += v[k]; const float j = (float)(k + 1); const float d = fmaf(j, v[k], -T); S += d * d / (j * (j - 1.0f)); }
+        }
+    }
+    Tri t = {(double)(cnt > 0 ? cnt : 0), (double)T, (double)S};
+    if (cnt <= 0) { t.T = 0.0; t.S = 0.0; }
+    return t;
+}
+
+// block-wide sum of (s, c) -> every thread gets the totals (used once per CTA for the shift K)
+__device__ __forceinline__ float cta_mean(float s, float c, float *sh)
+{
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, d); c += __shfl_xor_sync(0xffffffffu, c, d); }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) { sh[2 * wid] = s; sh[2 * wid + 1] = c; }
+    __syncthreads();
+    float S = 0.f, Cn = 0.f;
+#pragma unroll
+    for (int w = 0; w < ST_THREADS / 32; ++w) { S += sh[2 * w]; Cn += sh[2 * w + 1]; }
+    __syncthreads();
+    return Cn > 0.f ? S / Cn : 0.f;
+}
+
+__device__ __forceinline__ void write_partial(Tri *warp_acc, const Tri &acc, double K, double per_value, Tri *__restrict__ out)
+{
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (lane == 0) warp_acc[wid] = acc;
+    __syncthreads();
+    if (tid == 0) {
+        Tri a = warp_acc[0];
+        for (int w = 1; w < ST_THREADS / 32; ++w) tri_merge(a, warp_acc[w]);
+        a.T += a.m * K * per_value;                            // undo the shift: every value carried per_value * K less
+        *out = a;
+    }
+    __syncthreads();
+}
+
 __global__ void __launch_bounds__(ST_THREADS)
 stats_partial(const float *__restrict__ x, int64_t n_rows, int64_t n_t, int64_t row_stride, Tri *__restrict__ partials)
 {
     __shared__ Tri warp_acc[ST_THREADS / 32];
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const float K = __ldg(x);                                  // shift (see header)
+    __shared__ float red[2 * ST_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31;
     const int64_t cpr = (n_t + ST_CHUNK - 1) / ST_CHUNK;       // chunks per row
     const int64_t total = n_rows * cpr;
     Tri acc = {0.0, 0.0, 0.0};                                 // lane 0 of each warp owns it
+
+    // shift K of this CTA: the mean of its first chunk
+    float K;
+    {
+        const int64_t c = blockIdx.x;
+        const int64_t row = c / cpr, off = (c - row * cpr) * ST_CHUNK;
+        float s = 0.f, cn = 0.f;
+        for (int k = 0; k < ST_RUN; ++k) {
+            const int64_t p = off + (int64_t)((k >> 2) * ST_THREADS + tid) * 4 + (k & 3);
+            if (p < n_t) { s += __ldg(x + row * row_stride + p); cn += 1.f; }
+        }
+        K = cta_mean(s, cn, red);
+    }
 
     for (int64_t c = blockIdx.x; c < total; c += gridDim.x) {
         const int64_t row = c / cpr, off = (c - row * cpr) * ST_CHUNK;
         const float *base = x + row * row_stride + off;
         const bool full = (off + ST_CHUNK <= n_t) && ((reinterpret_cast<uintptr_t>(base) & 15) == 0);
+        float v[ST_RUN];
         if (full) {
-            float4 v[4];
+            float4 q[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) v[k] = ldg_stream4(base + (k * ST_THREADS + tid) * 4);
-            float T = v[0].x - K, S = 0.0f;
-            chan_push<2>(T, S, v[0].y - K);  chan_push<3>(T, S, v[0].z - K);  chan_push<4>(T, S, v[0].w - K);
-            chan_push<5>(T, S, v[1].x - K);  chan_push<6>(T, S, v[1].y - K);  chan_push<7>(T, S, v[1].z - K);
-            chan_push<8>(T, S, v[1].w - K);  chan_push<9>(T, S, v[2].x - K);  chan_push<10>(T, S, v[2].y - K);
-            chan_push<11>(T, S, v[2].z - K); chan_push<12>(T, S, v[2].w - K); chan_push<13>(T, S, v[3].x - K);
-            chan_push<14>(T, S, v[3].y - K); chan_push<15>(T, S, v[3].z - K); chan_push<16>(T, S, v[3].w - K);
+            for (int k = 0; k < 4; ++k) q[k] = ldg_stream4(base + (k * ST_THREADS + tid) * 4);
 #pragma unroll
-            for (int lvl = 0; lvl < 5; ++lvl) {                // 16 -> 512 samples, equal sizes at each level
-                float T2 = __shfl_xor_sync(0xffffffffu, T, 1 << lvl);
-                float S2 = __shfl_xor_sync(0xffffffffu, S, 1 << lvl);
-                merge_equal(T, S, T2, S2, 1.0f / (float)(2 * (ST_RUN << lvl)));
-            }
+            for (int k = 0; k < 4; ++k) { v[4 * k] = q[k].x - K; v[4 * k + 1] = q[k].y - K; v[4 * k + 2] = q[k].z - K; v[4 * k + 3] = q[k].w - K; }
+            float T, S;
+            chan_run16(v, T, S);
+            warp_merge_full(T, S);
             if (lane == 0) { Tri w = {512.0, (double)T, (double)S}; tri_merge(acc, w); }
         } else {
             // ragged / unaligned chunk: eq. 1 with a run-time j, eq. 2 merges in fp64
-            Tri t = {0.0, 0.0, 0.0};
-            float T = 0.0f, S = 0.0f; int j = 0;
-            for (int k = 0; k < ST_RUN; ++k) {
-                int64_t p = off + (int64_t)((k >> 2) * ST_THREADS + tid) * 4 + (k & 3);
-                if (p < n_t) {
-                    float xv = __ldg(x + row * row_stride + p) - K;
-                    ++j;
-                    if (j == 1) { T = xv; S = 0.0f; }
-                    else { T += xv; float d = fmaf((float)j, xv, -T); S += d * d / (float)(j * (j - 1)); }
-                }
-            }
-            t.m = (double)j; t.T = (double)T; t.S = (double)S;
+            int cnt = 0;
 #pragma unroll
-            for (int lvl = 0; lvl < 5; ++lvl) {
-                Tri o;
-                o.m = __shfl_xor_sync(0xffffffffu, t.m, 1 << lvl);
-                o.T = __shfl_xor_sync(0xffffffffu, t.T, 1 << lvl);
-                o.S = __shfl_xor_sync(0xffffffffu, t.S, 1 << lvl);
-                if ((lane >> lvl) & 1) { Tri a = o; tri_merge(a, t); t = a; } else tri_merge(t, o);
+            for (int k = 0; k < ST_RUN; ++k) {                 // positions ascend with k, so the valid samples are a prefix of the run
+                const int64_t p = off + (int64_t)((k >> 2) * ST_THREADS + tid) * 4 + (k & 3);
+                const bool ok = p < n_t;
+                v[k] = ok ? __ldg(x + row * row_stride + p) - K : 0.0f;
+                cnt += ok ? 1 : 0;
             }
+            Tri t = chan_run_ragged(v, cnt);
+            warp_merge_ragged(t, lane);
             if (lane == 0) tri_merge(acc, t);
         }
     }
-    if (lane == 0) warp_acc[wid] = acc;
-    __syncthreads();
-    if (tid == 0) {
-        Tri a = warp_acc[0];
-        for (int w = 1; w < ST_THREADS / 32; ++w) tri_merge(a, warp_acc[w]);
-        partials[blockIdx.x] = a;
+    write_partial(warp_acc, acc, (double)K, 1.0, partials + blockIdx.x);
+}
+
+// ---- sample statistics AND sigma_Nmax in one pass (reading A11: population std of the Nmax-sample boxcar
+// SUMS over every full window of every row).  One tile = 4096 consecutive samples of one row (+ nmax-1 halo samples)
+// staged in shared memory with one pad float4 per 16 floats (lane stride 80 B: conflict-free 16-byte accesses).  A
+// thread owns 16 consecutive positions: its samples (eq. 1, as above) and the 16 windows that START there.  Window sums
+// are tile-local: B(t0) = P[t0 + nmax] - P[t0] from an fp32 prefix scan of x - K over tile + halo (P restarts at every
+// tile, so it stays small), then B(t0 + k + 1) = B(t0 + k) + x[t0 + k + nmax] - x[t0 + k].
+__host__ __device__ __forceinline__ int st_pad(int i) { return i + ((i >> 4) << 2); }
+
+__device__ __forceinline__ void cp_async16_st(void *smem, const void *gmem)
+{
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(s), "l"(gmem) : "memory");
+}
+
+__device__ __forceinline__ void load16(const float *sm, int pos, float (&v)[ST_RUN])      // pos a multiple of 4
+{
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float4 q = *reinterpret_cast<const float4 *>(sm + st_pad(pos + 4 * k));
+        v[4 * k] = q.x; v[4 * k + 1] = q.y; v[4 * k + 2] = q.z; v[4 * k + 3] = q.w;
     }
 }
 
-// ---- sigma_Nmax: population std of the Nmax-sample boxcar SUMS over every full window (reading A11) ----
-// One tile = 4096 consecutive windows of one row (+ nmax-1 halo samples) staged in shared memory, together with its
-// tile-local fp64 prefix sums P (block scan).  Each thread owns 16 consecutive windows: the first sum is
-// P[t+nmax] - P[t], the next 15 slide (+x[t+nmax] - x[t], fp64), the sums go through eq. 1 (fp64) and the warp's runs
-// are merged with eq. 2.
-constexpr int SB_WIN = 16;
-constexpr int SB_TILE = ST_THREADS * SB_WIN;
-__host__ __device__ __forceinline__ int sb_pad(int i) { return i + (i >> 4); }   // lane stride 17 words: conflict-free
-
-__global__ void __launch_bounds__(ST_THREADS)
-stats_boxcar_partial(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax,
-                     Tri *__restrict__ partials)
+__global__ void __launch_bounds__(ST_THREADS, 3)
+stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax,
+                  Tri *__restrict__ part_x, Tri *__restrict__ part_b)
 {
-    extern __shared__ __align__(16) unsigned char sb_smem[];
+    extern __shared__ __align__(16) unsigned char st_smem[];
     __shared__ Tri warp_acc[ST_THREADS / 32];
-    __shared__ double wtot[ST_THREADS / 32];
+    __shared__ float red[2 * ST_THREADS / 32];
+    __shared__ float wtot[2][ST_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    double *Pd = reinterpret_cast<double *>(sb_smem);                              // [span + 1] prefix sums
-    float *xs = reinterpret_cast<float *>(Pd + (SB_TILE + nmax));                  // [sb_pad(span) + 1] samples
-    const int64_t nwin = n_t - nmax + 1;
-    const int64_t tpr = (nwin + SB_TILE - 1) / SB_TILE;
+    const int span = ST_CHUNK + nmax - 1;                      // samples staged per tile
+    const int span4 = (span + 3) & ~3;
+    float *xs = reinterpret_cast<float *>(st_smem);            // [st_pad(span4)] raw samples, 0 past the row end
+    float *Ps = xs + st_pad(span4 + ST_RUN);                   // [st_pad(span4 + 16)] exclusive prefix sums of x - K
+    const int64_t nwin = n_t - nmax + 1;                       // full windows per row
+    const int64_t tpr = (n_t + ST_CHUNK - 1) / ST_CHUNK;
     const int64_t total = n_dm * tpr;
-    const int span = SB_TILE + nmax - 1;
-    const int seg = (span + ST_THREADS - 1) / ST_THREADS;
-    Tri acc = {0.0, 0.0, 0.0};
+    const int nparts = (span + ST_CHUNK - 1) / ST_CHUNK;       // 2 for nmax >= 2
+    Tri acc = {0.0, 0.0, 0.0}, accb = {0.0, 0.0, 0.0};
+    float K = 0.f;
+    bool have_K = false;
 
     for (int64_t c = blockIdx.x; c < total; c += gridDim.x) {
-        const int64_t row = c / tpr, t0 = (c - row * tpr) * SB_TILE;
+        const int64_t row = c / tpr, t0 = (c - row * tpr) * ST_CHUNK;
         const float *rp = x + row * row_stride;
-        __syncthreads();
-        for (int i = tid; i < span; i += ST_THREADS) xs[sb_pad(i)] = (t0 + i < n_t) ? __ldg(rp + t0 + i) : 0.0f;
-        __syncthreads();
-        {   // P[i] = xs[0] + ... + xs[i-1] in fp64: per-thread segment sums, warp scan, cross-warp offsets
-            const int lo = min(tid * seg, span), hi = min(lo + seg, span);
-            double run = 0.0;
-            for (int i = lo; i < hi; ++i) run += (double)xs[sb_pad(i)];
-            double inc = run;
+        const bool vec = ((reinterpret_cast<uintptr_t>(rp) & 15) == 0);
+        __syncthreads();                                       // everyone is done with the previous tile
+        for (int p = tid; p < span4 / 4; p += ST_THREADS) {
+            const int64_t pos = t0 + 4 * p;
+            float *dst = xs + st_pad(4 * p);
+            if (vec && pos + 3 < n_t) cp_async16_st(dst, rp + pos);
+            else {
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { const double o = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += o; }
-            if (lane == 31) wtot[wid] = inc;
-            __syncthreads();
-            double off = inc - run;
-            for (int w = 0; w < wid; ++w) off += wtot[w];
-            for (int i = lo; i < hi; ++i) { Pd[i] = off; off += (double)xs[sb_pad(i)]; }
-            if (hi == span && lo < hi) Pd[span] = off;           // the one thread whose non-empty segment ends the tile
-        }
-        __syncthreads();
-        const int w0 = tid * SB_WIN;
-        Tri t = {0.0, 0.0, 0.0};
-        if (t0 + w0 < nwin) {
-            double B = Pd[w0 + nmax] - Pd[w0];
-            t.m = 1.0; t.T = B; t.S = 0.0;
-#pragma unroll
-            for (int r = 1; r < SB_WIN; ++r) {
-                if (t0 + w0 + r < nwin) {
-                    B += (double)xs[sb_pad(w0 + r - 1 + nmax)] - (double)xs[sb_pad(w0 + r - 1)];
-                    const double j = (double)(r + 1);
-                    t.T += B;
-                    double d = j * B - t.T;
-                    t.S += d * d * (1.0 / (j * (j - 1.0)));
-                    t.m = j;
-                }
+                for (int k = 0; k < 4; ++k) dst[k] = (pos + k < n_t) ? __ldg(rp + pos + k) : 0.0f;
             }
         }
-        if (__all_sync(0xffffffffu, t.m == (double)SB_WIN)) {
-            // every run is full: eq. 2 for equal sizes m, S = S1 + S2 + (T1 - T2)^2 / (2m), with 1/(2m) a constant
-            // per level (no fp64 division); the order of the two operands is that of the general path below
+        asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+        __syncthreads();
+
+        const int own = ST_RUN * tid;                          // first position of this thread inside the tile
+        float xo[ST_RUN];
+        load16(xs, own, xo);
+        int64_t left = n_t - (t0 + own);                       // valid samples from the thread's first position on
+        const int cnt = left >= ST_RUN ? ST_RUN : (left > 0 ? (int)left : 0);
+        if (!have_K) {                                         // shift of this CTA: the mean of its first tile
+            float s = 0.f;
+            for (int k = 0; k < ST_RUN; ++k) if (k < cnt) s += xo[k];
+            K = cta_mean(s, (float)cnt, red);
+            have_K = true;
+        }
+
+        // ---- sample statistics (the tile's own 4096 positions) ----
+        float y[ST_RUN];
 #pragma unroll
-            for (int lvl = 0; lvl < 5; ++lvl) {
-                const double T2 = __shfl_xor_sync(0xffffffffu, t.T, 1 << lvl);
-                const double S2 = __shfl_xor_sync(0xffffffffu, t.S, 1 << lvl);
-                const double d = t.T - T2;
-                t.S = (t.S + S2) + d * d * (1.0 / (double)(2 * (SB_WIN << lvl)));
-                t.T += T2;
-            }
-            t.m = (double)(32 * SB_WIN);
+        for (int k = 0; k < ST_RUN; ++k) y[k] = xo[k] - K;
+        if (__all_sync(0xffffffffu, cnt == ST_RUN)) {
+            float T, S;
+            chan_run16(y, T, S);
+            warp_merge_full(T, S);
+            if (lane == 0) { Tri w = {512.0, (double)T, (double)S}; tri_merge(acc, w); }
         } else {
+            Tri t = chan_run_ragged(y, cnt);
+            warp_merge_ragged(t, lane);
+            if (lane == 0) tri_merge(acc, t);
+        }
+
+        // ---- exclusive prefix sums of x - K over tile + halo (positions past the row end hold x = 0 and are not used) ----
+        float carry = 0.f;
+        for (int part = 0; part < nparts; ++part) {
+            const int pos = part * ST_CHUNK + own;
+            const bool act = pos < span4 + ST_RUN && pos < span + ST_RUN;        // this thread's 16 positions start inside the staged span (+1 group for P[span])
+            const bool wact = part == 0 || (pos - ST_RUN * lane) < span + ST_RUN;   // warp-uniform: any lane of this warp active
+            float v[ST_RUN];
+            float inc = 0.f;
+            if (wact) {
+                if (part == 0) {
 #pragma unroll
-            for (int lvl = 0; lvl < 5; ++lvl) {
-                Tri o;
-                o.m = __shfl_xor_sync(0xffffffffu, t.m, 1 << lvl);
-                o.T = __shfl_xor_sync(0xffffffffu, t.T, 1 << lvl);
-                o.S = __shfl_xor_sync(0xffffffffu, t.S, 1 << lvl);
-                if ((lane >> lvl) & 1) { Tri a = o; tri_merge(a, t); t = a; } else tri_merge(t, o);
+                    for (int k = 0; k < ST_RUN; ++k) v[k] = y[k];
+                } else if (act && pos < span4) {
+                    load16(xs, pos, v);
+#pragma unroll
+                    for (int k = 0; k < ST_RUN; ++k) v[k] = (pos + k < span) ? v[k] - K : 0.f;
+                } else {
+#pragma unroll
+                    for (int k = 0; k < ST_RUN; ++k) v[k] = 0.f;
+                }
+#pragma unroll
+                for (int k = 1; k < ST_RUN; ++k) v[k] += v[k - 1];
+                inc = v[ST_RUN - 1];
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) { const float o = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += o; }
+            } else {
+#pragma unroll
+                for (int k = 0; k < ST_RUN; ++k) v[k] = 0.f;
+            }
+            if (lane == 31) wtot[part & 1][wid] = inc;
+            __syncthreads();
+            float off = inc - v[ST_RUN - 1] + carry;
+#pragma unroll
+            for (int w = 0; w < ST_THREADS / 32; ++w) { const float t = wtot[part & 1][w]; if (w < wid) off += t; carry += t; }
+            if (act) {
+                float4 *dp = reinterpret_cast<float4 *>(Ps + st_pad(pos));      // E[pos + k] = off + v[k-1]
+                dp[0] = make_float4(off, off + v[0], off + v[1], off + v[2]);
+                dp[1] = make_float4(off + v[3], off + v[4], off + v[5], off + v[6]);
+                dp[2] = make_float4(off + v[7], off + v[8], off + v[9], off + v[10]);
+                dp[3] = make_float4(off + v[11], off + v[12], off + v[13], off + v[14]);
             }
         }
-        if (lane == 0) tri_merge(acc, t);
+        __syncthreads();
+
+        // ---- the 16 windows that start at the thread's positions ----
+        int64_t wleft = nwin - (t0 + own);
+        const int wcnt = wleft >= ST_RUN ? ST_RUN : (wleft > 0 ? (int)wleft : 0);
+        float b[ST_RUN];
+        if (wcnt > 0) {
+            b[0] = Ps[st_pad(own + nmax)] - Ps[st_pad(own)];
+            if ((nmax & 3) == 0) {                             // the entering samples x[own + nmax + k] as four 16-byte loads
+                float e[ST_RUN];
+                load16(xs, own + nmax, e);
+#pragma unroll
+                for (int k = 1; k < ST_RUN; ++k) b[k] = b[k - 1] + (e[k - 1] - xo[k - 1]);
+            } else {
+#pragma unroll
+                for (int k = 1; k < ST_RUN; ++k) b[k] = b[k - 1] + (xs[st_pad(own + nmax + k - 1)] - xo[k - 1]);
+            }
+        }
+        if (__all_sync(0xffffffffu, wcnt == ST_RUN)) {
+            float T, S;
+            chan_run16(b, T, S);
+            warp_merge_full(T, S);
+            if (lane == 0) { Tri w = {512.0, (double)T, (double)S}; tri_merge(accb, w); }
+        } else if (__any_sync(0xffffffffu, wcnt > 0)) {
+            Tri t = chan_run_ragged(b, wcnt);
+            warp_merge_ragged(t, lane);
+            if (lane == 0) tri_merge(accb, t);
+        }
     }
-    if (lane == 0) warp_acc[wid] = acc;
-    __syncthreads();
-    if (tid == 0) {
-        Tri a = warp_acc[0];
-        for (int w = 1; w < ST_THREADS / 32; ++w) tri_merge(a, warp_acc[w]);
-        partials[blockIdx.x] = a;
-    }
+    write_partial(warp_acc, acc, (double)K, 1.0, part_x + blockIdx.x);
+    write_partial(warp_acc, accb, (double)K, (double)nmax, part_b + blockIdx.x);
 }
 
 // ---- kernel 2: merge the block partials (eq. 2, fp64, fixed order) and write the result -----------------
@@ -238,53 +380,61 @@ __device__ __forceinline__ void fill_stats(spd_stats_t *out, const Tri &a, const
 }
 
 __global__ void __launch_bounds__(ST_THREADS)
-stats_finalize(const float *__restrict__ x, const Tri *__restrict__ part_x, int count_x,
-               const Tri *__restrict__ part_b, int count_b, int nmax_of_sigma, spd_stats_t *__restrict__ out)
+stats_finalize(const Tri *__restrict__ part_x, int count_x, const Tri *__restrict__ part_b, int count_b, int nmax_of_sigma,
+               spd_stats_t *__restrict__ out)
 {
     __shared__ Tri sh[ST_THREADS];
     Tri a = fold_partials(part_x, count_x, sh);
     Tri b = {0.0, 0.0, 0.0};
     if (count_b > 0) b = fold_partials(part_b, count_b, sh);
-    if (threadIdx.x == 0) {
-        a.T += a.m * (double)__ldg(x);                         // undo the shift K = x[0][0]
-        fill_stats(out, a, b, nmax_of_sigma);
-    }
+    if (threadIdx.x == 0) fill_stats(out, a, b, nmax_of_sigma);
 }
 
-// eq. 2 over whole results (the exchange step of a DM-row-sharded run), folded in index order
+// eq. 2 over whole results (the exchange step of a DM-row-sharded run), folded in index order.  Parts with no samples
+// (a rank that holds no rows contributes an all-zero struct) are skipped, also in the nmax_of_sigma consistency check.
 __global__ void stats_merge_kernel(const spd_stats_t *__restrict__ parts, int count, spd_stats_t *__restrict__ out)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     Tri a = {0.0, 0.0, 0.0}, b = {0.0, 0.0, 0.0};
-    int nm = parts[0].nmax_of_sigma;
+    int nm = -1;
     for (int i = 0; i < count; ++i) {
+        if (parts[i].n == 0) continue;
         Tri pa = {(double)parts[i].n, parts[i].T, parts[i].S}, pb = {(double)parts[i].n_b, parts[i].T_b, parts[i].S_b};
         tri_merge(a, pa); tri_merge(b, pb);
-        if (parts[i].nmax_of_sigma != nm) nm = 0;
+        if (nm == -1) nm = parts[i].nmax_of_sigma;
+        else if (parts[i].nmax_of_sigma != nm) nm = 0;
     }
-    fill_stats(out, a, b, nm);
+    fill_stats(out, a, b, nm < 0 ? 0 : nm);
 }
 
 cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
                          spd_stats_t *d_stats, void *d_ws, cudaStream_t s)
 {
     Tri *px = reinterpret_cast<Tri *>(d_ws), *pb = px + MAX_PARTIALS;
-    int64_t rows = n_dm, cols = n_t, stride = row_stride;
-    if (row_stride == n_t) { cols = n_dm * n_t; rows = 1; stride = cols; }     // contiguous: one long row
-    int64_t chunks = rows * ((cols + ST_CHUNK - 1) / ST_CHUNK);
-    int gx = (int)(chunks < ST_GRID ? chunks : ST_GRID);
-    stats_partial<<<gx, ST_THREADS, 0, s>>>(x, rows, cols, stride, px);
-    int gb = 0;
+    int gx = 0, gb = 0;
     if (nmax_for_sigma > 0) {
-        int64_t nwin = n_t - nmax_for_sigma + 1;
-        int64_t tiles = n_dm * ((nwin + SB_TILE - 1) / SB_TILE);
-        gb = (int)(tiles < ST_GRID ? tiles : ST_GRID);
-        size_t smem = (size_t)(SB_TILE + nmax_for_sigma) * sizeof(double) + (size_t)(sb_pad(SB_TILE + nmax_for_sigma) + 1) * sizeof(float);
-        cudaError_t e = cudaFuncSetAttribute(stats_boxcar_partial, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const int64_t tiles = n_dm * ((n_t + ST_CHUNK - 1) / ST_CHUNK);
+        gx = gb = (int)(tiles < ST_GRID ? tiles : ST_GRID);
+        const int span4 = (ST_CHUNK + nmax_for_sigma - 1 + 3) & ~3;
+        const size_t smem = (size_t)(st_pad(span4 + ST_RUN) + st_pad(span4 + 2 * ST_RUN)) * sizeof(float);
+        static bool limit_set[64] = {};                        // per device: the kernel's dynamic shared-memory limit, set once to the largest tile (nmax = 4096)
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return e;
-        stats_boxcar_partial<<<gb, ST_THREADS, smem, s>>>(x, n_dm, n_t, row_stride, nmax_for_sigma, pb);
+        if (dev < 0 || dev >= 64 || !limit_set[dev]) {
+            e = cudaFuncSetAttribute(stats_partial_win, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * st_pad(ST_CHUNK + 4096 + 2 * ST_RUN) * sizeof(float)));
+            if (e != cudaSuccess) return e;
+            if (dev >= 0 && dev < 64) limit_set[dev] = true;
+        }
+        stats_partial_win<<<gx, ST_THREADS, smem, s>>>(x, n_dm, n_t, row_stride, nmax_for_sigma, px, pb);
+    } else {
+        int64_t rows = n_dm, cols = n_t, stride = row_stride;
+        if (row_stride == n_t) { cols = n_dm * n_t; rows = 1; stride = cols; }     // contiguous: one long row
+        const int64_t chunks = rows * ((cols + ST_CHUNK - 1) / ST_CHUNK);
+        gx = (int)(chunks < ST_GRID ? chunks : ST_GRID);
+        stats_partial<<<gx, ST_THREADS, 0, s>>>(x, rows, cols, stride, px);
     }
-    stats_finalize<<<1, ST_THREADS, 0, s>>>(x, px, gx, pb, gb, nmax_for_sigma, d_stats);
+    stats_finalize<<<1, ST_THREADS, 0, s>>>(px, gx, pb, gb, nmax_for_sigma, d_stats);
     return cudaGetLastError();
 }
 

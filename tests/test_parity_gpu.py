@@ -69,6 +69,20 @@ def test_sigma_nmax_parity(P, shape, nmax):
         assert r, str(r)
 
 
+@pytest.mark.parametrize("where", [(0, 0), (0, 4095), (2, 7000), (3, 12287)])
+@pytest.mark.parametrize("nmax", [0, 64])
+def test_stats_with_one_huge_outlier(P, where, nmax):
+    """A single 1e4-sigma sample (bright RFI) must not cost the fp32 chunks their digits: the shift K of a CTA is the
+    mean of its first chunk, not one sample (VERDICT r1 weak #6: the old K = x[0][0] was fragile)."""
+    from gpu_util import gpu_stats
+    x = (100.0 + 20.0 * rng(104).standard_normal((4, 12288))).astype(np.float32)
+    x[where] = 100.0 + 20.0 * 1e4
+    g, _ = gpu_stats(x, nmax)
+    o = O.full_stats(x, nmax)
+    r = CMP.compare_stats(float(g["mean"]), float(g["sigma"]), o, float(g["sigma_nmax"]) if nmax else None)
+    assert r, str(r)
+
+
 def test_stats_is_bit_reproducible(P):
     from gpu_util import gpu_stats
     x = (100 + 20 * rng(102).standard_normal((64, 16384))).astype(np.float32)
@@ -87,6 +101,21 @@ def test_stats_merge_equals_whole(P):
     m = P.read_stats(P.spd_stats_merge(parts, 3))[0]
     o = O.full_stats(x, 16)
     assert int(m["n"]) == x.size and int(m["n_b"]) == 10 * (6000 - 15)
+    r = CMP.compare_stats(float(m["mean"]), float(m["sigma"]), o, float(m["sigma_nmax"]))
+    assert r, str(r)
+
+
+def test_stats_merge_skips_empty_parts(P):
+    """A rank that holds no rows contributes an all-zero struct: eq. 2 skips it, also in the nmax_of_sigma check."""
+    from gpu_util import to_dev
+    x = (3.0 + rng(105).standard_normal((6, 5000))).astype(np.float32)
+    parts = P.new_stats(count=3)
+    nb = P.STATS_DTYPE.itemsize
+    P.spd_stats(to_dev(x[0:4]), 32, stats=parts[0:nb])
+    P.spd_stats(to_dev(x[4:6]), 32, stats=parts[2 * nb:3 * nb])            # the middle part stays all-zero
+    m = P.read_stats(P.spd_stats_merge(parts, 3))[0]
+    o = O.full_stats(x, 32)
+    assert int(m["n"]) == x.size and int(m["nmax_of_sigma"]) == 32
     r = CMP.compare_stats(float(m["mean"]), float(m["sigma"]), o, float(m["sigma_nmax"]))
     assert r, str(r)
 
@@ -262,14 +291,17 @@ def test_candidates_ragged_and_strided(P):
 _ORACLE_STATS = {}
 
 
-def _whole_path(P, cfg, x, nmax, rows=None, fused=True):
-    """stats -> sweep -> candidates on the GPU; oracle on all rows, or on `rows` with the ORACLE's full-array stats."""
+def _whole_path(P, cfg, x, nmax, rows=None, fused=True, block=256, tie_rate_max=0.05):
+    """stats -> sweep -> candidates on the GPU over the WHOLE array (the launch configuration bench.py times); the oracle on
+    all rows, or on `rows`, with the ORACLE's full-array statistics, streamed in blocks of <= `block` rows so that neither
+    side's planes are ever wholly on the host (SURVEY.md 8(d) "Oracle timed beside it")."""
     from gpu_util import gpu_candidates, gpu_fused
     d = torch.from_numpy(x).cuda()
     mode = cfg.sigma_mode
     st = P.spd_stats(d, nmax if mode != "sqrt" else 0)
     snr, width = P.spd_boxcar_snr(d, st, nmax, mode)
     rec, total = gpu_candidates(snr, width, cfg.threshold, capacity=1 << 22)
+    assert total <= 1 << 22
     g = P.read_stats(st)[0]
     key = (cfg.cid, x.shape, nmax if mode != "sqrt" else 0)
     if key not in _ORACLE_STATS:                       # the float64 stream over 2^31 samples takes ~30 s: once per config
@@ -278,21 +310,8 @@ def _whole_path(P, cfg, x, nmax, rows=None, fused=True):
     r = CMP.compare_stats(float(g["mean"]), float(g["sigma"]), o, float(g["sigma_nmax"]) if mode != "sqrt" else None)
     assert r, str(r)
     sig = O.sigma_table(o.sigma, o.sigma_nmax, nmax, mode)
-    sel = np.arange(x.shape[0]) if rows is None else np.asarray(sorted(rows))
-    xs = np.ascontiguousarray(x[sel])
-    o_snr, o_w, o_m = O.sweep(xs, o.mean, sig)
-    idx = torch.from_numpy(sel).cuda()
-    g_snr = snr[idx].cpu().numpy()
-    g_w = width.view(torch.int16)[idx].cpu().numpy().view(np.uint16)      # uint16 has no index kernel in torch
-    r = CMP.compare_planes(xs, o.mean, sig, g_snr, g_w, o_snr, o_w, o_m)
-    assert r, str(r)
-    # candidates restricted to the compared rows
-    pos = {int(s): i for i, s in enumerate(sel)}
-    m = np.isin(rec["dm"], sel)
-    dm_local = np.array([pos[int(v)] for v in rec["dm"][m]], dtype=np.int64)
-    rc = CMP.compare_candidates(dm_local, rec["t"][m], rec["snr"][m], rec["width"][m], int(m.sum()), 1 << 22,
-                                o_snr, o_w, o_m, cfg.threshold, xs, o.mean, sig)
-    assert rc, str(rc)
+    sel_all = np.arange(x.shape[0]) if rows is None else np.asarray(sorted(rows))
+    rec2 = None
     if fused:
         # the fused kernel takes the width by replaying the running sums, the plane kernel from a prefix sum: the
         # records agree in (dm, t, snr) bit for bit and in width outside near-ties; against the oracle both obey the rules
@@ -302,18 +321,36 @@ def _whole_path(P, cfg, x, nmax, rows=None, fused=True):
         for k in ("dm", "t", "snr"):
             assert a[k].tobytes() == b[k].tobytes(), k
         assert (a["width"] != b["width"]).mean() <= 2e-3
-        m2 = np.isin(rec2["dm"], sel)
-        dm2 = np.array([pos[int(v)] for v in rec2["dm"][m2]], dtype=np.int64)
-        rc2 = CMP.compare_candidates(dm2, rec2["t"][m2], rec2["snr"][m2], rec2["width"][m2], int(m2.sum()), 1 << 22,
-                                     o_snr, o_w, o_m, cfg.threshold, xs, o.mean, sig)
-        assert rc2, str(rc2)
-    return rec, total, r, rc
+    info = {"rows": int(sel_all.size), "oracle_hits": 0, "gpu_hits": 0, "near_tie_exempt": 0, "near_threshold_exempt": 0, "samples": 0}
+    for lo in range(0, sel_all.size, block):
+        sel = sel_all[lo:lo + block]
+        xs = np.ascontiguousarray(x[sel])
+        o_snr, o_w, o_m = O.sweep(xs, o.mean, sig)
+        idx = torch.from_numpy(sel).cuda()
+        g_snr = snr[idx].cpu().numpy()
+        g_w = width.view(torch.int16)[idx].cpu().numpy().view(np.uint16)      # uint16 has no index kernel in torch
+        r = CMP.compare_planes(xs, o.mean, sig, g_snr, g_w, o_snr, o_w, o_m)
+        assert r, f"rows {sel[0]}..{sel[-1]}: {r}"
+        assert r.info["near_tie_rate"] < tie_rate_max  # far above the expected 0.3-2 % (eq. 4 on noise) would be a bug, not a tie
+        pos = np.full(x.shape[0], -1, dtype=np.int64)
+        pos[sel] = np.arange(sel.size)
+        for which in ([rec] if rec2 is None else [rec, rec2]):
+            m = pos[which["dm"]] >= 0                  # candidates restricted to the compared rows
+            rc = CMP.compare_candidates(pos[which["dm"][m]], which["t"][m], which["snr"][m], which["width"][m], int(m.sum()), 1 << 22,
+                                        o_snr, o_w, o_m, cfg.threshold, xs, o.mean, sig)
+            assert rc, f"rows {sel[0]}..{sel[-1]}: {rc}"
+        info["oracle_hits"] += rc.info["oracle_hits"]; info["gpu_hits"] += int(m.sum())
+        info["near_tie_exempt"] += r.info["width_near_tie_exempt"]; info["near_threshold_exempt"] += rc.info["near_threshold_exempt"]
+        info["samples"] += xs.size
+    if rows is None:                                   # every row was compared: the whole-array hit count is the oracle's, up to the exempted samples
+        assert abs(total - info["oracle_hits"]) <= info["near_threshold_exempt"]
+    return rec, total, info
 
 
 def test_config1_whole_path(P):
     cfg = gen.get_config(1)
     x = gen.make_array(cfg)
-    rec, total, r, rc = _whole_path(P, cfg, x, cfg.nmax[0])
+    rec, total, info = _whole_path(P, cfg, x, cfg.nmax[0])
     for p in gen.pulse_table(cfg):                     # every injected pulse is recovered at (about) its width
         sel = (rec["dm"] == p.row) & (np.abs(rec["t"].astype(np.int64) - p.start) <= cfg.nmax[0])
         assert sel.any(), p
@@ -321,39 +358,48 @@ def test_config1_whole_path(P):
         assert abs(rec["snr"][k] - p.snr) < 3.0 and 0.5 * p.width <= rec["width"][k] <= 2 * p.width + 1
 
 
-def test_config2_whole_path_full_size(P):
+def test_config2_whole_path_every_row(P):
+    """BASELINE config 2 (1024 x 131072, mu = 100, sigma = 20, Nmax 64): every row against the oracle."""
     cfg = gen.get_config(2)
     x = gen.make_array(cfg)
-    rows = sorted(set(gen.pulse_rows(cfg)) | set(range(0, cfg.n_dm, 64)))
-    _whole_path(P, cfg, x, cfg.nmax[0], rows=rows)
+    _, total, info = _whole_path(P, cfg, x, cfg.nmax[0])
+    assert info["rows"] == cfg.n_dm and info["samples"] == x.size
 
 
-def _sample_rows(cfg, every, n_pulse_rows):
-    """Every `every`-th row plus the first `n_pulse_rows` pulse-bearing rows (sampled outputs at full size)."""
-    return sorted(set(range(0, cfg.n_dm, every)) | set(gen.pulse_rows(cfg)[:n_pulse_rows]) | {cfg.n_dm - 1})
+def _survey_rows(cfg, cap_pulse_rows):
+    """every 16th row plus every pulse-bearing row and its +-3 neighbours, the latter capped."""
+    pulse = []
+    for r in gen.pulse_rows(cfg):
+        pulse += [q for q in range(r - 3, r + 4) if 0 <= q < cfg.n_dm]
+    pulse = sorted(set(pulse))[:cap_pulse_rows]
+    return sorted(set(range(0, cfg.n_dm, 16)) | set(pulse) | {cfg.n_dm - 1})
 
 
-def test_config3_whole_path_full_size_sampled_rows(P):
-    """BASELINE config 3 (SKA-like, 6000 x 262144, Nmax 128) in the launch configuration bench.py times: stats on the
-    full array; planes and candidates on sampled rows, each compared element by element with the oracle."""
+def test_config3_whole_path_every_row(P):
+    """BASELINE config 3 (SKA-like, 6000 x 262144, Nmax 128) in the launch configuration bench.py times: statistics, both
+    planes and the candidate list of EVERY row against the oracle, streamed in 256-row blocks (~1 min of oracle time)."""
     cfg = gen.get_config(3)
     x = gen.make_array(cfg)
-    _whole_path(P, cfg, x, cfg.nmax[0], rows=_sample_rows(cfg, 400, 24))
+    _, total, info = _whole_path(P, cfg, x, cfg.nmax[0])
+    assert info["rows"] == cfg.n_dm and info["samples"] == x.size and total > 0
 
 
-def test_config4_eq5_whole_path_full_size_sampled_rows(P):
-    """BASELINE config 4 (signal-dominated, eq. 5 literal with the measured sigma_Nmax, Nmax 512)."""
+def test_config4_eq5_whole_path_survey_rows(P):
+    """BASELINE config 4 (signal-dominated, eq. 5 literal with the measured sigma_Nmax, Nmax 512): statistics on the full
+    array; planes and candidates on every 16th row plus the pulse-bearing rows +-3 (capped at 192)."""
     cfg = gen.get_config(4)
     x = gen.make_array(cfg)
-    _whole_path(P, cfg, x, cfg.nmax[0], rows=_sample_rows(cfg, 256, 8))
+    # eq. 5 as printed flattens the SNR over the wide widths (sigma_N grows ~linearly), so near-ties are more frequent here (~5 %)
+    _whole_path(P, cfg, x, cfg.nmax[0], rows=_survey_rows(cfg, 192), tie_rate_max=0.10)
 
 
 @pytest.mark.parametrize("nmax", [8, 32, 128, 512])
-def test_config5_width_sweep_full_size_sampled_rows(P, nmax):
-    """BASELINE config 5 (4096 x 524288 = 2^31 samples: every flat offset must be 64-bit) at each Nmax of the sweep."""
+def test_config5_width_sweep_survey_rows(P, nmax):
+    """BASELINE config 5 (4096 x 524288 = 2^31 samples: every flat offset must be 64-bit) at each Nmax of the sweep: every
+    16th row plus pulse-bearing rows +-3 (capped at 64)."""
     cfg = gen.get_config(5)
     x = _c5_array(cfg)
-    _whole_path(P, cfg, x, nmax, rows=_sample_rows(cfg, 1024, 6), fused=(nmax == 32))
+    _whole_path(P, cfg, x, nmax, rows=_survey_rows(cfg, 64), fused=(nmax == 32))
 
 
 _C5 = {}
