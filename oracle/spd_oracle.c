@@ -15,7 +15,10 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): P1 two-pass numpy mean/std, P2 closed
  * forms, P3 eq.2 merge-order invariance, P4 rectangular-pulse closed form (Figure 1),
  * P5 constant input (tie-break + row-end rule), P6 brute-force O(n*Nmax^2) inner sums,
- * P7 pure-noise normalisation, P8 sigma table end points, P9 candidate set = brute filter.
+ * P7 pure-noise normalisation, P8 sigma table end points, P9 candidate set = brute filter,
+ * P10 (tests/test_oracle_decimated.py) for O5, decimation in time + boxcar: level 0 = O3, decimated
+ * series = block sums, every level = explicit sums over the original samples, on-grid pulse = A sqrt(W),
+ * off-grid sensitivity >= sqrt(0.9).
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -223,4 +226,59 @@ int64_t spd_oracle_candidates(const double *snr, const int32_t *width, int64_t n
             }
         }
     return count;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O5  decimation in time + boxcar for wide filters  (section 3: "we will use a
+ * combination of boxcar filtering with the decimation in time of the input data")
+ *
+ * The paper names the route but gives no algorithm; this is reading A20 of DESIGN.md, written out
+ * step by step.  It is an APPROXIMATION of the exhaustive search O3: the width grid gets coarser
+ * with width (PAPER.md:21, :69 warn about the sensitivity this costs).
+ *
+ *   level 0:  x_0 = x.  Boxcars of every width w' = 1..W0 at every sample: exactly O3 with Nmax = W0.
+ *   level l:  x_l[i] = x_{l-1}[2i] + x_{l-1}[2i+1],  i < n_l = floor(n_{l-1} / 2)      (decimation by 2)
+ *             boxcars of widths w' = W0/2+1 .. W0 (in decimated samples) at every decimated sample i;
+ *             one of them covers N = w' 2^l samples of x starting at t = i 2^l, so
+ *                 SNR = (B - N mu) / sigma_N      with sigma_N from O2 for the EFFECTIVE width N
+ *             (mu, sigma are those of x: nothing is re-measured per level).  Widths
+ *             w' <= W0/2 are left to the finer levels, which cover them at twice the resolution.
+ *   Only widths that fit are evaluated (reading A9): w' <= n_l - i.  A position where none of the
+ *   level's widths fits gets snr = -inf, width = 0.
+ *
+ * This function does ONE level on an already decimated row block xl (float64, [n_dm][n_l]):
+ *   lvl = l, sig[N-1] = sigma_N for N = 1..W0 2^l, wmin = smallest width evaluated (1 at level 0, W0/2+1 above).
+ * Outputs per decimated sample: snr, width = EFFECTIVE width N (0 if none), margin = best - second.  */
+void spd_oracle_sweep_level(const double *xl, int64_t n_dm, int64_t n_l, double mu, const double *sig,
+                            int w0, int wmin, int lvl, double *snr, int32_t *width, double *margin)
+{
+    const int64_t D = (int64_t)1 << lvl;
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        const double *row = xl + d * n_l;
+        for (int64_t i = 0; i < n_l; ++i) {
+            double B = 0.0, best = -INFINITY, second = -INFINITY;
+            int32_t W = 0;
+            int64_t wmax = n_l - i < (int64_t)w0 ? n_l - i : (int64_t)w0;
+            for (int64_t w = 1; w <= wmax; ++w) {
+                B += row[i + w - 1];
+                if (w < wmin) continue;
+                int64_t N = w * D;
+                double s = (B - (double)N * mu) / sig[N - 1];
+                if (s > best) { second = best; best = s; W = (int32_t)N; }
+                else if (s > second) second = s;
+            }
+            int64_t o = d * n_l + i;
+            snr[o] = best; width[o] = W; margin[o] = best - second;
+        }
+    }
+}
+
+/* x_l[i] = x_{l-1}[2i] + x_{l-1}[2i+1] for one level (float64 in, float64 out, [n_dm][n_prev] -> [n_dm][n_prev/2]) */
+void spd_oracle_decimate2(const double *xp, int64_t n_dm, int64_t n_prev, double *xl)
+{
+    const int64_t n_l = n_prev / 2;
+    for (int64_t d = 0; d < n_dm; ++d)
+        for (int64_t i = 0; i < n_l; ++i)
+            xl[d * n_l + i] = xp[d * n_prev + 2 * i] + xp[d * n_prev + 2 * i + 1];
 }

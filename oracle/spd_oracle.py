@@ -49,6 +49,10 @@ def _load():
         L.spd_oracle_sweep.argtypes = [P, i64, i64, i64, dbl, P, i32, P, P, P]
         L.spd_oracle_snr_fixed_width.argtypes = [P, i64, i64, i64, dbl, dbl, i32, P]
         L.spd_oracle_snr_at.argtypes = [P, i64, i64, dbl, P, i32, P, P, P, i64, P]
+        L.spd_oracle_sweep_level.argtypes = [P, i64, i64, dbl, P, i32, i32, i32, P, P, P]
+        L.spd_oracle_sweep_level.restype = None
+        L.spd_oracle_decimate2.argtypes = [P, i64, i64, P]
+        L.spd_oracle_decimate2.restype = None
         L.spd_oracle_candidates.argtypes = [P, P, i64, i64, dbl, i64, P, P, P, P]
         L.spd_oracle_candidates.restype = i64
         for f in ("spd_oracle_stats", "spd_oracle_merge", "spd_oracle_chan_run", "spd_oracle_sigma_nmax",
@@ -169,6 +173,38 @@ def candidates(snr: np.ndarray, width: np.ndarray, f_T: float):
     c_snr = np.empty(cnt, dtype=np.float64); c_w = np.empty(cnt, dtype=np.int32)
     L.spd_oracle_candidates(_p(snr), _p(width), n_dm, n_t, float(f_T), cnt, _p(c_dm), _p(c_t), _p(c_snr), _p(c_w))
     return c_dm, c_t, c_snr, c_w
+
+
+def decimated_levels(w0: int, levels: int):
+    """Width grid of O5: [(level, decimation 2^l, smallest w', largest w')]; Nmax = w0 * 2^(levels-1)."""
+    assert w0 >= 2 and w0 % 2 == 0 and levels >= 1
+    return [(l, 1 << l, 1 if l == 0 else w0 // 2 + 1, w0) for l in range(levels)]
+
+
+def sweep_decimated(x: np.ndarray, mu: float, sigma: float, sig_nmax: float, mode, w0: int, levels: int):
+    """O5 (reading A20): decimation in time + boxcar.  Returns one dict per level:
+    {level, D, x (float64 decimated rows), snr, width (effective, 0 = no width fits), margin, sig (sigma_N, N = 1..w0*D)}.
+    sigma_N is that of the exhaustive search of the SAME Nmax = w0 * 2^(levels-1) (eq. 4 / eq. 5 / anchored)."""
+    x, n_dm, n_t, rs = _as_x(x)
+    nmax = w0 * (1 << (levels - 1))
+    sig_all = sigma_table(sigma, sig_nmax, nmax, mode)
+    L = _load()
+    cur = np.ascontiguousarray(x[:, :n_t], dtype=np.float64)
+    out = []
+    for lvl, D, wmin, wmax in decimated_levels(w0, levels):
+        if lvl > 0:
+            nxt = np.empty((n_dm, cur.shape[1] // 2), dtype=np.float64)
+            L.spd_oracle_decimate2(_p(cur), n_dm, cur.shape[1], _p(nxt))
+            cur = nxt
+        n_l = cur.shape[1]
+        snr = np.empty((n_dm, n_l), dtype=np.float64)
+        width = np.empty((n_dm, n_l), dtype=np.int32)
+        margin = np.empty((n_dm, n_l), dtype=np.float64)
+        sig = np.ascontiguousarray(sig_all[: w0 * D])
+        if n_l > 0:
+            L.spd_oracle_sweep_level(_p(cur), n_dm, n_l, float(mu), _p(sig), int(w0), int(wmin), int(lvl), _p(snr), _p(width), _p(margin))
+        out.append(dict(level=lvl, D=D, x=cur, snr=snr, width=width, margin=margin, sig=sig))
+    return out
 
 
 def search(x: np.ndarray, nmax: int, mode="sqrt", f_T: float = 6.0):
