@@ -113,6 +113,34 @@ spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t
                             spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,
                             void *d_ws, size_t ws_bytes, void *stream);
 
+/* Decimation in time + boxcar for wide filters (section 3: "a combination of boxcar filtering with the
+ * decimation in time of the input data"; the paper names the route, the algorithm is reading A20 of DESIGN.md).
+ * An APPROXIMATION of spd_boxcar_snr with nmax = w0 * 2^(levels-1): the width grid gets coarser with width
+ * (PAPER.md:21, :69 warn about the sensitivity this costs: at most 1 - sqrt(0.9) = 5.1 % for w0 = 16).
+ *   level 0: every width 1..w0 at every sample (exactly spd_boxcar_snr with nmax = w0);
+ *   level l: x_l[i] = x_{l-1}[2i] + x_{l-1}[2i+1] (n_l = n_t >> l samples per row), widths w' = w0/2+1..w0 of x_l at every
+ *            decimated sample i: effective width N = w' 2^l, start sample t = i 2^l,
+ *            SNR = (B - N mu) / sigma_N with sigma_N of the exhaustive search of the same nmax (eq. 4 / eq. 5 / anchored).
+ * Planes are packed per row: level l occupies elements [spd_decimated_level_offset(n_t, l), + n_l) of a row of
+ * plane_stride elements (>= spd_decimated_level_offset(n_t, levels), a multiple of 8).  d_width holds the EFFECTIVE width
+ * N; a position where none of the level's widths fits has snr = -inf, width = 0.
+ * Requires w0 in {16, 32}, 1 <= levels <= 8, w0 <= n_t, w0 * 2^(levels-1) <= 4096.  d_ws: >= spd_decimated_workspace_bytes()
+ * bytes, 256-byte aligned (it holds the decimated series of two levels at a time).  LINEAR modes need d_stats measured
+ * with nmax_for_sigma = w0 * 2^(levels-1). */
+int64_t spd_decimated_level_offset(int64_t n_t, int level);
+size_t spd_decimated_workspace_bytes(int64_t n_dm, int64_t n_t, int w0, int levels);
+spd_status spd_boxcar_snr_decimated(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                                    const spd_stats_t *d_stats, int w0, int levels, spd_sigma_mode mode,
+                                    float *d_snr, uint16_t *d_width, int64_t plane_stride,
+                                    void *d_ws, size_t ws_bytes, void *stream);
+
+/* Candidate selection over the packed planes of spd_boxcar_snr_decimated: one list for all levels,
+ * record.t = start sample in the ORIGINAL series (i 2^l), record.width = effective width.  A pulse is usually reported by
+ * several levels (the list is unordered and not clustered).  *d_count / capacity follow spd_candidates. */
+spd_status spd_candidates_decimated(const float *d_snr, const uint16_t *d_width, int64_t n_dm, int64_t n_t, int64_t plane_stride,
+                                    int levels, float threshold, spd_candidate_t *d_out, uint64_t capacity,
+                                    unsigned long long *d_count, void *stream);
+
 /* Device bytes spd_search_host needs in d_arena for this shape and capacity. */
 size_t spd_search_host_arena_bytes(int64_t n_dm, int64_t n_t, int nmax, uint64_t capacity);
 

@@ -105,6 +105,57 @@ def compare_planes(x: np.ndarray, mu: float, sig: np.ndarray,
     return r
 
 
+def compare_planes_level(x: np.ndarray, mu: float, sig_all: np.ndarray, w0: int, level: dict,
+                         g_snr: np.ndarray, g_width: np.ndarray) -> Report:
+    """One level of the decimated search (oracle O5, `level` = one dict of spd_oracle.sweep_decimated) against the GPU's
+    plane of that level.  Same rules as compare_planes; in addition a position where none of the level's widths fits must
+    be (-inf, 0) on both sides, and a width reported inside a near-tie must lie on the level's grid (a multiple of
+    D = 2^l with w0/2 < N/D <= w0, or 1 <= N <= w0 at level 0) and is re-summed over the ORIGINAL samples x."""
+    r = Report()
+    D, lvl = int(level["D"]), int(level["level"])
+    o_snr, o_width, o_margin = level["snr"], level["width"], level["margin"]
+    g_snr = np.asarray(g_snr, dtype=np.float64)
+    g_width = np.asarray(g_width).astype(np.int64)
+    if g_snr.shape != o_snr.shape or g_width.shape != o_width.shape:
+        r.fail(f"shape {g_snr.shape}/{g_width.shape} vs {o_snr.shape}")
+        return r
+    none = o_width == 0
+    if np.any(g_width[none] != 0) or np.any(g_snr[none] != -np.inf):
+        r.fail(f"{int(np.count_nonzero((g_width != 0) & none))} positions where no width of the level fits are not (-inf, 0)")
+    ok = ~none
+    if np.any(g_width[ok] == 0) or not np.all(np.isfinite(g_snr[ok])):
+        r.fail("GPU reports no width / a non-finite SNR where the level has widths that fit")
+        return r
+    d = np.abs(g_snr[ok] - o_snr[ok])
+    bad = d > np.maximum(SNR_ABS, SNR_REL * np.abs(o_snr[ok]))
+    r.info["snr_max_abs_err"] = float(d.max()) if d.size else 0.0
+    r.info["snr_violations"] = int(bad.sum())
+    if bad.any():
+        r.fail(f"level {lvl} SNR: {int(bad.sum())} samples out of tolerance")
+    mism = ok & (g_width != o_width)
+    hard = mism & (o_margin > TIE)
+    r.info["width_mismatch"] = int(mism.sum())
+    if hard.any():
+        i = np.argwhere(hard)[0]
+        r.fail(f"level {lvl} width: {int(hard.sum())} mismatches outside near-ties, first at {tuple(i)}: "
+               f"{int(g_width[tuple(i)])} vs {int(o_width[tuple(i)])}")
+    soft = mism & ~(o_margin > TIE)
+    r.info["width_near_tie_exempt"] = int(soft.sum())
+    r.info["near_tie_rate"] = float(np.count_nonzero(ok & ~(o_margin > TIE))) / max(1, int(ok.sum()))
+    if soft.any():
+        idx = np.argwhere(soft)
+        N = g_width[soft]
+        wp = N // D
+        on_grid = (N % D == 0) & (wp <= w0) & (wp >= (1 if lvl == 0 else w0 // 2 + 1)) & (idx[:, 1] + wp <= o_snr.shape[1])
+        s_at = O.snr_at(x, mu, sig_all, idx[:, 0], idx[:, 1] * D, N.astype(np.int32))
+        worse = ~on_grid | ~(np.abs(s_at - o_snr[soft]) <= TIE)
+        if worse.any():
+            k = int(np.argmax(worse))
+            r.fail(f"level {lvl} width: {int(worse.sum())} near-tie widths off the grid or not within {TIE} of best, first at "
+                   f"{tuple(idx[k])}: width {int(N[k])}")
+    return r
+
+
 def compare_candidates(g_dm, g_t, g_snr, g_width, g_count: int, capacity: int,
                        o_snr: np.ndarray, o_width: np.ndarray, o_margin: np.ndarray,
                        f_T: float, x: np.ndarray, mu: float, sig: np.ndarray) -> Report:

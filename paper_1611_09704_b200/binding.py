@@ -52,7 +52,12 @@ def lib() -> C.CDLL:
         L.spd_search_fused.argtypes = [vp, i64, i64, i64, vp, i32, i32, f32, vp, u64, vp, vp, sz, vp]
         L.spd_search_host_arena_bytes.argtypes = [i64, i64, i32, u64]; L.spd_search_host_arena_bytes.restype = sz
         L.spd_search_host.argtypes = [vp, i64, i64, i32, i32, f32, vp, u64, vp, vp, vp, sz, vp]
-        for f in ("spd_stats", "spd_stats_merge", "spd_boxcar_snr", "spd_candidates", "spd_search_fused", "spd_search_host"):
+        L.spd_decimated_level_offset.argtypes = [i64, i32]; L.spd_decimated_level_offset.restype = i64
+        L.spd_decimated_workspace_bytes.argtypes = [i64, i64, i32, i32]; L.spd_decimated_workspace_bytes.restype = sz
+        L.spd_boxcar_snr_decimated.argtypes = [vp, i64, i64, i64, vp, i32, i32, i32, vp, vp, i64, vp, sz, vp]
+        L.spd_candidates_decimated.argtypes = [vp, vp, i64, i64, i64, i32, f32, vp, u64, vp, vp]
+        for f in ("spd_stats", "spd_stats_merge", "spd_boxcar_snr", "spd_candidates", "spd_search_fused", "spd_search_host",
+                  "spd_boxcar_snr_decimated", "spd_candidates_decimated"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -158,6 +163,47 @@ def spd_search_fused(x: torch.Tensor, stats: torch.Tensor, nmax: int, mode, thre
     _check(lib().spd_search_fused(x.data_ptr(), n_dm, n_t, rs, stats.data_ptr(), int(nmax), _MODES[mode], float(threshold),
                                   out.data_ptr(), out.shape[0], count.data_ptr(), ws.data_ptr(), ws.numel(),
                                   _stream(stream)), "spd_search_fused")
+    return out, count
+
+
+def decimated_level_offset(n_t: int, level: int) -> int:
+    """First element of level `level` inside a row of the packed planes; level == levels gives the row length."""
+    return int(lib().spd_decimated_level_offset(n_t, level))
+
+
+def spd_boxcar_snr_decimated(x: torch.Tensor, stats: torch.Tensor, w0: int, levels: int, mode="sqrt",
+                             snr: Optional[torch.Tensor] = None, width: Optional[torch.Tensor] = None,
+                             ws: Optional[torch.Tensor] = None, stream=None):
+    """Decimation in time + boxcar (include/spd.h): returns the packed (snr f32, width u16) planes [n_dm][plane_stride];
+    level l of row d is [d, decimated_level_offset(n_t, l) : + (n_t >> l)]."""
+    n_dm, n_t, rs = _plane(x, torch.float32, "x")
+    stride = decimated_level_offset(n_t, levels)
+    if stride < 0:
+        raise SpdError("spd_boxcar_snr_decimated: invalid n_t / levels")
+    if snr is None:
+        snr = torch.empty((n_dm, stride), dtype=torch.float32, device=x.device)
+    if width is None:
+        width = torch.empty((n_dm, stride), dtype=torch.uint16, device=x.device)
+    if _plane(snr, torch.float32, "snr") != _plane(width, torch.uint16, "width") or snr.shape[0] != n_dm:
+        raise SpdError("packed snr / width planes must share one shape and row stride")
+    need = int(lib().spd_decimated_workspace_bytes(n_dm, n_t, int(w0), int(levels)))
+    if need == 0:
+        raise SpdError("spd_boxcar_snr_decimated: w0 must be 16 or 32, 1 <= levels <= 8, w0 * 2^(levels-1) <= 4096")
+    ws = torch.empty(need, dtype=torch.uint8, device=x.device) if ws is None else ws
+    _check(lib().spd_boxcar_snr_decimated(x.data_ptr(), n_dm, n_t, rs, stats.data_ptr(), int(w0), int(levels), _MODES[mode],
+                                          snr.data_ptr(), width.data_ptr(), snr.stride(0), ws.data_ptr(), ws.numel(),
+                                          _stream(stream)), "spd_boxcar_snr_decimated")
+    return snr, width
+
+
+def spd_candidates_decimated(snr: torch.Tensor, width: torch.Tensor, n_t: int, levels: int, threshold: float,
+                             out: Optional[torch.Tensor] = None, count: Optional[torch.Tensor] = None,
+                             capacity: int = 1 << 20, stream=None):
+    n_dm, _, stride = _plane(snr, torch.float32, "snr")
+    if out is None or count is None:
+        out, count = new_candidates(capacity, snr.device)
+    _check(lib().spd_candidates_decimated(snr.data_ptr(), width.data_ptr(), n_dm, int(n_t), stride, int(levels), float(threshold),
+                                          out.data_ptr(), out.shape[0], count.data_ptr(), _stream(stream)), "spd_candidates_decimated")
     return out, count
 
 

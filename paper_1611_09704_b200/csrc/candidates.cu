@@ -26,7 +26,7 @@ __global__ void zero_count_kernel(unsigned long long *count) { *count = 0ULL; }
 __global__ void __launch_bounds__(CD_THREADS)
 candidates_compact(const float *__restrict__ snr, const uint16_t *__restrict__ width, int64_t n_dm, int64_t n_t,
                    int64_t row_stride, float thr, spd_candidate_t *__restrict__ out, unsigned long long capacity,
-                   unsigned long long *__restrict__ count)
+                   unsigned long long *__restrict__ count, uint32_t t_scale /* record.t = t_scale * sample index (decimated levels) */)
 {
     const int tid = threadIdx.x;
     const int64_t cpr = (n_t + CD_CHUNK - 1) / CD_CHUNK;
@@ -65,7 +65,7 @@ candidates_compact(const float *__restrict__ snr, const uint16_t *__restrict__ w
                     const bool hit = v[k][e] >= thr;
                     uint32_t w = 0;
                     if (hit && width) w = width[row * row_stride + p];
-                    append_candidate(hit, (uint32_t)row, (uint32_t)p, v[k][e], w, out, capacity, count);
+                    append_candidate(hit, (uint32_t)row, (uint32_t)p * t_scale, v[k][e], w, out, capacity, count);
                 }
         }
     }
@@ -73,13 +73,14 @@ candidates_compact(const float *__restrict__ snr, const uint16_t *__restrict__ w
 
 cudaError_t launch_candidates(const float *snr, const uint16_t *width, int64_t n_dm, int64_t n_t, int64_t row_stride,
                               float threshold, spd_candidate_t *out, unsigned long long capacity,
-                              unsigned long long *d_count, cudaStream_t s)
+                              unsigned long long *d_count, cudaStream_t s, bool zero_count, uint32_t t_scale)
 {
-    zero_count_kernel<<<1, 1, 0, s>>>(d_count);
+    if (zero_count) zero_count_kernel<<<1, 1, 0, s>>>(d_count);
     int64_t rows = n_dm, cols = n_t, stride = row_stride;
     const int64_t chunks = rows * ((cols + CD_CHUNK - 1) / CD_CHUNK);
     const int g = (int)(chunks < CD_GRID ? chunks : CD_GRID);
-    candidates_compact<<<g, CD_THREADS, 0, s>>>(snr, width, rows, cols, stride, threshold, out, capacity, d_count);
+    if (chunks <= 0) return cudaGetLastError();
+    candidates_compact<<<g, CD_THREADS, 0, s>>>(snr, width, rows, cols, stride, threshold, out, capacity, d_count, t_scale);
     return cudaGetLastError();
 }
 

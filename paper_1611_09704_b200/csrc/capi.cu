@@ -106,6 +106,85 @@ spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t
     return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
 }
 
+// ---- decimation in time + boxcar (reading A20) ----------------------------------------------------
+namespace {
+inline bool dec_ok(int w0, int levels, int64_t n_t) { return (w0 == 16 || w0 == 32) && levels >= 1 && levels <= 8 && (int64_t)w0 <= n_t && (w0 << (levels - 1)) <= NMAX_API_LIMIT; }
+inline int64_t dec_n(int64_t n_t, int l) { return n_t >> l; }
+inline int64_t dec_off(int64_t n_t, int l) { int64_t o = 0; for (int k = 0; k < l; ++k) o += (dec_n(n_t, k) + 7) & ~(int64_t)7; return o; }
+inline int64_t dec_stride(int64_t n_l) { return (n_l + 3) & ~(int64_t)3; }            // row stride of a decimated series in the workspace
+}
+
+int64_t spd_decimated_level_offset(int64_t n_t, int level)
+{
+    if (n_t < 1 || level < 0 || level > 8) return -1;
+    return dec_off(n_t, level);                                  // level == levels gives the elements per row of the packed planes
+}
+
+size_t spd_decimated_workspace_bytes(int64_t n_dm, int64_t n_t, int w0, int levels)
+{
+    if (n_dm < 1 || n_t < 1 || !dec_ok(w0, levels, n_t)) return 0;
+    size_t b = align_up(spd_workspace_bytes(n_dm, n_t, w0), 256) + 256;            // sigma table + one spd_stats_t for the level
+    if (levels > 1) b += align_up((size_t)n_dm * (size_t)dec_stride(dec_n(n_t, 1)) * 4, 256);
+    if (levels > 2) b += align_up((size_t)n_dm * (size_t)dec_stride(dec_n(n_t, 2)) * 4, 256);
+    return b;
+}
+
+spd_status spd_boxcar_snr_decimated(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                                    const spd_stats_t *d_stats, int w0, int levels, spd_sigma_mode mode,
+                                    float *d_snr, uint16_t *d_width, int64_t plane_stride,
+                                    void *d_ws, size_t ws_bytes, void *stream)
+{
+    if (!d_x || !d_stats || !d_snr || !d_width || !d_ws || !shape_ok(n_dm, n_t, row_stride) || !dec_ok(w0, levels, n_t))
+        return SPD_ERR_INVALID_ARG;
+    if ((int)mode < 0 || (int)mode > 2 || (reinterpret_cast<uintptr_t>(d_ws) & 255) != 0) return SPD_ERR_INVALID_ARG;
+    if (plane_stride < dec_off(n_t, levels) || (plane_stride & 7) != 0) return SPD_ERR_INVALID_ARG;
+    if (ws_bytes < spd_decimated_workspace_bytes(n_dm, n_t, w0, levels)) return SPD_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    unsigned char *p = reinterpret_cast<unsigned char *>(d_ws);
+    float *table = reinterpret_cast<float *>(p);                  p += align_up(spd_workspace_bytes(n_dm, n_t, w0), 256);
+    spd_stats_t *lst = reinterpret_cast<spd_stats_t *>(p);        p += 256;
+    float *buf[2] = {nullptr, nullptr};
+    if (levels > 1) { buf[0] = reinterpret_cast<float *>(p); p += align_up((size_t)n_dm * (size_t)dec_stride(dec_n(n_t, 1)) * 4, 256); }
+    if (levels > 2) { buf[1] = reinterpret_cast<float *>(p); }
+    const int nmax_total = w0 << (levels - 1);
+    const bool rc = sweep_uses_constant_table(w0, (int)mode);
+    const float *src = d_x;
+    int64_t src_stride = row_stride;
+    for (int l = 0; l < levels; ++l) {
+        const int D = 1 << l;
+        const int64_t n_l = dec_n(n_t, l);
+        if (l > 0) {                                              // x_l = pairwise sums of x_{l-1}; the two buffers alternate
+            float *dst = buf[(l - 1) & 1];
+            const int64_t dst_stride = dec_stride(n_l);
+            if (launch_decimate2(src, n_dm, n_l, src_stride, dst, dst_stride, s) != cudaSuccess) return SPD_ERR_CUDA;
+            src = dst; src_stride = dst_stride;
+        }
+        if (n_l < 1) break;
+        if (launch_level_stats(d_stats, D, lst, s) != cudaSuccess) return SPD_ERR_CUDA;
+        if (!rc && launch_sigma_table(d_stats, w0, (int)mode, table, s, D, nmax_total) != cudaSuccess) return SPD_ERR_CUDA;
+        const int64_t off = dec_off(n_t, l);
+        if (launch_sweep_level(src, n_dm, n_l, src_stride, lst, table, w0, l == 0 ? 0 : w0 / 2, D, rc, d_snr + off, d_width + off,
+                               plane_stride, s) != cudaSuccess) return SPD_ERR_CUDA;
+    }
+    return SPD_OK;
+}
+
+spd_status spd_candidates_decimated(const float *d_snr, const uint16_t *d_width, int64_t n_dm, int64_t n_t, int64_t plane_stride,
+                                    int levels, float threshold, spd_candidate_t *d_out, uint64_t capacity,
+                                    unsigned long long *d_count, void *stream)
+{
+    if (!d_snr || !d_width || !d_count || (!d_out && capacity > 0) || n_dm < 1 || n_t < 1 || levels < 1 || levels > 8)
+        return SPD_ERR_INVALID_ARG;
+    if (threshold != threshold || plane_stride < dec_off(n_t, levels)) return SPD_ERR_INVALID_ARG;
+    for (int l = 0; l < levels; ++l) {
+        const int64_t off = dec_off(n_t, l), n_l = dec_n(n_t, l);
+        if (n_l < 1) break;
+        if (launch_candidates(d_snr + off, d_width + off, n_dm, n_l, plane_stride, threshold, d_out, capacity, d_count,
+                              (cudaStream_t)stream, l == 0, 1u << l) != cudaSuccess) return SPD_ERR_CUDA;
+    }
+    return SPD_OK;
+}
+
 // arena layout of spd_search_host: x | candidates | stats | count | workspace
 size_t spd_search_host_arena_bytes(int64_t n_dm, int64_t n_t, int nmax, uint64_t capacity)
 {

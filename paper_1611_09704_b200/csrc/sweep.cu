@@ -109,27 +109,77 @@ __device__ __forceinline__ void cp_async_commit_wait_all()
 
 // r_w = 1/sigma_w for w = 1..nmax: eq. 4, eq. 5 as printed, or the anchored variant.
 // fp64 throughout, rounded once to fp32.  LINEAR modes fed stats measured for another Nmax write NaN.
-__global__ void sigma_table_kernel(const spd_stats_t *__restrict__ st, int nmax, int mode, float *__restrict__ table)
+// Decimated levels (spd_boxcar_snr_decimated): entry w' - 1 holds 1/sigma_N of the EFFECTIVE width N = w' * wscale, with
+// sigma_N of the exhaustive search of nmax_total = the widest effective width (st holds the statistics of the ORIGINAL x).
+__global__ void sigma_table_kernel(const spd_stats_t *__restrict__ st, int nmax, int mode, float *__restrict__ table,
+                                   int wscale, int nmax_total)
 {
     const double sigma = st->sigma, snm = st->sigma_nmax;
-    const bool bad = (mode != SPD_SIGMA_SQRT) && (st->nmax_of_sigma != nmax);
+    const bool bad = (mode != SPD_SIGMA_SQRT) && (st->nmax_of_sigma != nmax_total);
     for (int w = 1 + blockIdx.x * blockDim.x + threadIdx.x; w <= sw_rt_len(nmax); w += gridDim.x * blockDim.x) {
         float r = __int_as_float(0x7fc00000);      // widths past nmax (padding of the last block of 8) never win
         if (w <= nmax) {
-            double s = sqrt((double)w) * sigma;
-            if (mode == SPD_SIGMA_LINEAR && nmax > 1) s += (double)(w - 1) * snm / (double)(nmax - 1);
-            if (mode == SPD_SIGMA_LINEAR_ANCHORED && nmax > 1)
-                s += (double)(w - 1) * (snm - sqrt((double)nmax) * sigma) / (double)(nmax - 1);
+            const double N = (double)w * (double)wscale;
+            double s = sqrt(N) * sigma;
+            if (mode == SPD_SIGMA_LINEAR && nmax_total > 1) s += (N - 1.0) * snm / (double)(nmax_total - 1);
+            if (mode == SPD_SIGMA_LINEAR_ANCHORED && nmax_total > 1)
+                s += (N - 1.0) * (snm - sqrt((double)nmax_total) * sigma) / (double)(nmax_total - 1);
             r = bad ? __int_as_float(0x7fc00000) : (float)(1.0 / s);
         }
         table[w - 1] = r;
     }
 }
 
-cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, float *d_table, cudaStream_t s)
+cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, float *d_table, cudaStream_t s, int wscale, int nmax_total)
 {
     int n = sw_rt_len(nmax);
-    sigma_table_kernel<<<(n + 255) / 256, 256, 0, s>>>(d_stats, nmax, mode, d_table);
+    sigma_table_kernel<<<(n + 255) / 256, 256, 0, s>>>(d_stats, nmax, mode, d_table, wscale, nmax_total > 0 ? nmax_total : nmax);
+    return cudaGetLastError();
+}
+
+// ---- decimation in time (reading A20): x_l[i] = x_{l-1}[2i] + x_{l-1}[2i+1]; the statistics of a level are those
+// of x scaled to sums of D = 2^l samples: mean_l = D mu, sigma_l = sqrt(D) sigma (eq. 3), so that eq. 4 of the decimated
+// series at width w' IS eq. 4 of x at the effective width w' D.  Nothing is re-measured.
+__global__ void decimate2_kernel(const float *__restrict__ src, int64_t n_dm, int64_t n_l, int64_t src_stride,
+                                 float *__restrict__ dst, int64_t dst_stride)
+{
+    const int64_t q4 = (n_l + 3) / 4;                           // groups of 4 outputs per row
+    const int64_t total = n_dm * q4;
+    for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t row = g / q4, i = (g - row * q4) * 4;
+        const float *sp = src + row * src_stride + 2 * i;
+        float *dp = dst + row * dst_stride + i;
+        if (i + 3 < n_l && ((reinterpret_cast<uintptr_t>(sp) & 15) == 0) && ((reinterpret_cast<uintptr_t>(dp) & 15) == 0)) {
+            float4 a, b;
+            asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w) : "l"(sp));
+            asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w) : "l"(sp + 4));
+            *reinterpret_cast<float4 *>(dp) = make_float4(__fadd_rn(a.x, a.y), __fadd_rn(a.z, a.w), __fadd_rn(b.x, b.y), __fadd_rn(b.z, b.w));
+        } else {
+            for (int k = 0; k < 4 && i + k < n_l; ++k) dp[k] = __fadd_rn(__ldg(sp + 2 * k), __ldg(sp + 2 * k + 1));
+        }
+    }
+}
+
+__global__ void level_stats_kernel(const spd_stats_t *__restrict__ st, int D, spd_stats_t *__restrict__ out)
+{
+    spd_stats_t s = *st;
+    s.mean = st->mean * (double)D;
+    s.sigma = st->sigma * sqrt((double)D);
+    *out = s;
+}
+
+cudaError_t launch_decimate2(const float *src, int64_t n_dm, int64_t n_l, int64_t src_stride, float *dst, int64_t dst_stride, cudaStream_t s)
+{
+    const int64_t groups = n_dm * ((n_l + 3) / 4);
+    if (groups <= 0) return cudaSuccess;
+    const int64_t blocks = (groups + 255) / 256;
+    decimate2_kernel<<<(unsigned)(blocks < 148 * 16 ? blocks : 148 * 16), 256, 0, s>>>(src, n_dm, n_l, src_stride, dst, dst_stride);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_level_stats(const spd_stats_t *st, int D, spd_stats_t *out, cudaStream_t s)
+{
+    level_stats_kernel<<<1, 1, 0, s>>>(st, D, out);
     return cudaGetLastError();
 }
 
@@ -292,7 +342,7 @@ __device__ __forceinline__ void note_block(const float2 (&now)[SW_R], const floa
 
 // SNR (f32) and width (u16) of a thread's 8 + 8 samples: 16-byte streaming stores where the row is aligned and whole
 template <int SW_THREADS>
-__device__ __forceinline__ void store_planes(float *__restrict__ snr, uint16_t *__restrict__ width, int64_t row, int64_t row_stride,
+__device__ __forceinline__ void store_planes(float *__restrict__ snr, uint16_t *__restrict__ width, int64_t row, int64_t row_stride /* of the planes */,
                                              int64_t n_t, int64_t ta, const float2 (&best)[SW_R], const int (&wx)[SW_R], const int (&wy)[SW_R])
 {
     const int64_t tb = ta + SW_THREADS * SW_R;
@@ -646,7 +696,7 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
 // values closer than 32 ulp (4e-6 relative, far inside the 1e-3 tie tolerance of DESIGN.md section 5) may resolve
 // either way.  The SNR written is the exact maximum.  A tagged -inf (a window past the row end) or NaN (a width past
 // nmax) is a NaN, which FMNMX drops.  No scan, no width search, no bookkeeping.
-template <int KB, bool RC>
+template <int KB, bool RC, bool EVAL>
 __device__ __forceinline__ void sweep8_tagged(float2 (&B)[SW_R], float2 (&W)[SW_R], float2 (&best)[SW_R], float2 (&tbest)[SW_R],
                                               const float2 *__restrict__ zp, const float *__restrict__ rp, int mask)
 {
@@ -663,6 +713,7 @@ __device__ __forceinline__ void sweep8_tagged(float2 (&B)[SW_R], float2 (&W)[SW_
             B[j] = __fadd2_rn(B[j], W[(j + u) & 7]);
             const float2 s0 = __fmul2_rn(B[j], r0);
             B[j] = __fadd2_rn(B[j], (j == SW_R - 1) ? n0 : W[(j + u + 1) & 7]);
+            if (!EVAL) continue;                   // a decimated level leaves its narrow widths to the finer levels: running sums only
             const float2 s1 = __fmul2_rn(B[j], r1);
             best[j].x = fmax3(best[j].x, s0.x, s1.x);
             best[j].y = fmax3(best[j].y, s0.y, s1.y);
@@ -678,7 +729,9 @@ template <int SW_THREADS, bool RC>
 __global__ void __launch_bounds__(SW_THREADS, 640 / SW_THREADS)
 boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                         const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
-                        float *__restrict__ snr, uint16_t *__restrict__ width)
+                        float *__restrict__ snr, uint16_t *__restrict__ width,
+                        int wmin /* widths <= wmin are summed but not evaluated (0 or a multiple of 8) */,
+                        int wscale /* reported width = w * wscale */, int64_t out_stride /* row stride of the planes */)
 {
     constexpr int SW_SUB = SW_THREADS * SW_R, SW_TILE = 2 * SW_SUB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -732,19 +785,29 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); tbest[j] = make_float2(NINF, NINF); }
         const float2 *zp = Z + 9 * (tid + 1);
-        sweep8_tagged<0, RC>(B, W, best, tbest, zp, rtf, mask31);
-        if (nblk > 1) sweep8_tagged<1, RC>(B, W, best, tbest, zp + 9, rtf + 8, mask31);
-        if (nblk > 2) sweep8_tagged<2, RC>(B, W, best, tbest, zp + 18, rtf + 16, mask31);
-        if (nblk > 3) sweep8_tagged<3, RC>(B, W, best, tbest, zp + 27, rtf + 24, mask31);
+        if (wmin >= 8) sweep8_tagged<0, RC, false>(B, W, best, tbest, zp, rtf, mask31);
+        else sweep8_tagged<0, RC, true>(B, W, best, tbest, zp, rtf, mask31);
+        if (nblk > 1) {
+            if (wmin >= 16) sweep8_tagged<1, RC, false>(B, W, best, tbest, zp + 9, rtf + 8, mask31);
+            else sweep8_tagged<1, RC, true>(B, W, best, tbest, zp + 9, rtf + 8, mask31);
+        }
+        if (nblk > 2) sweep8_tagged<2, RC, true>(B, W, best, tbest, zp + 18, rtf + 16, mask31);
+        if (nblk > 3) sweep8_tagged<3, RC, true>(B, W, best, tbest, zp + 27, rtf + 24, mask31);
 
         int wx[SW_R], wy[SW_R];
 #pragma unroll
-        for (int j = 0; j < SW_R; ++j) { wx[j] = 32 - (__float_as_int(tbest[j].x) & 31); wy[j] = 32 - (__float_as_int(tbest[j].y) & 31); }
+        for (int j = 0; j < SW_R; ++j) {
+            wx[j] = (32 - (__float_as_int(tbest[j].x) & 31)) * wscale; wy[j] = (32 - (__float_as_int(tbest[j].y) & 31)) * wscale;
+            if (wmin > 0) {                         // a position where none of the level's widths fits: snr = -inf, width = 0
+                if (best[j].x == NINF) wx[j] = 0;
+                if (best[j].y == NINF) wy[j] = 0;
+            }
+        }
         if (!RC && rtf[0] != rtf[0]) {              // NaN table (LINEAR mode fed stats of another Nmax) must surface
 #pragma unroll
             for (int j = 0; j < SW_R; ++j) { best[j] = make_float2(rtf[0], rtf[0]); wx[j] = 1; wy[j] = 1; }
         }
-        store_planes<SW_THREADS>(snr, width, row, row_stride, n_t, T0 + SW_R * tid, best, wx, wy);
+        store_planes<SW_THREADS>(snr, width, row, out_stride, n_t, T0 + SW_R * tid, best, wx, wy);
     }
     cp_async_commit_wait_all();
 }
@@ -816,7 +879,8 @@ static cudaError_t launch_sweep_nt(const float *x, int64_t n_dm, int64_t n_t, in
     } else if (nmax <= SW_NARROW_NMAX) {
         const FusedSmem lay(nmax, NT);
         if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep_narrow<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
+        boxcar_snr_sweep_narrow<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width,
+                                                                    0, 1, row_stride);
     } else {
         const SweepSmem lay(nmax, NT);
         if ((e = persistent_grid(boxcar_snr_sweep<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
@@ -837,6 +901,28 @@ cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
     }
     if (rc) return launch_sweep_nt<128, true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
     return launch_sweep_nt<128, false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
+}
+
+// one level of the decimated search: the narrow kernel on the decimated series x_l (w0 <= 32) with the level's statistics
+cudaError_t launch_sweep_level(const float *xl, int64_t n_dm, int64_t n_l, int64_t xl_stride, const spd_stats_t *d_stats_level,
+                               const float *d_table, int w0, int wmin, int wscale, bool rc, float *snr, uint16_t *width,
+                               int64_t out_stride, cudaStream_t s)
+{
+    constexpr int NT = 64, TILE = 2 * NT * SW_R;
+    if (n_l <= 0) return cudaSuccess;
+    const int tpr = (int)((n_l + TILE - 1) / TILE);
+    const int64_t tiles = n_dm * (int64_t)tpr;
+    const FusedSmem lay(w0, NT);
+    unsigned grid = 0;
+    cudaError_t e;
+    if (rc) {
+        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, true>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep_narrow<NT, true><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride);
+    } else {
+        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, false>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep_narrow<NT, false><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride);
+    }
+    return cudaGetLastError();
 }
 
 }  // namespace spd

@@ -28,12 +28,12 @@ __device__ __forceinline__ float fmax3(float a, float b, float c) { return fmaxf
 
 enum Mode { FADD, FMUL, FFMA, FMNMX, FMNMX3, FADD2, FMUL2, FMUL2_BCAST, FFMA2, MIX_SCALAR, MIX_SCALAR_RCONST, MIX_PACKED, MIX_PACKED_RCONST, MIX_PACKED_RCONST_ARGMAX, NMODES };
 static const char *mode_name[NMODES] = {
-    "FADD  r,r", "FMUL  r,r", "FFMA  r,r,r", "FMNMX r,r", "FMNMX3 r,r,r", "FADD2 rr,rr", "FMUL2 rr,rr", "FMUL2 rr,r (scalar broadcast)",
+    "FADD  r,r", "FMUL  r,r", "FFMA  r,r,r", "FMNMX r,r x2 (ptxas fuses two into one FMNMX3)", "FMNMX3 r,r,r", "FADD2 rr,rr", "FMUL2 rr,rr", "FMUL2 rr,r (scalar broadcast)",
     "FFMA2 rr,rr,rr", "loop mix, scalar: 2 FADD + 2 FMUL + 1 FMNMX3 per 2 pairs", "loop mix, scalar, r_w from the constant bank",
     "loop mix, packed: 2 FADD2 + 2 FMUL2(bcast) + 2 FMNMX3 per 4 pairs", "loop mix, packed, r_w from the constant bank (uniform register)",
     "loop mix, packed, r_w constant, + block arg-max (ping-pong maxima, FSETP + SEL per sum per 8 widths)"};
 // warp instructions per repetition, and (sample, width) pairs per repetition per lane (0 = not a loop mix)
-static const int mode_instr[NMODES] = {16, 16, 16, 16, 16, 8, 8, 8, 8, 40, 40, 48, 48, 112};
+static const int mode_instr[NMODES] = {16, 16, 16, 8, 16, 8, 8, 8, 8, 40, 40, 48, 48, 112};
 static const int mode_pairs[NMODES] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 16, 16, 32, 32, 64};
 
 struct RTable { float r[8]; };

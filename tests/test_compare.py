@@ -218,3 +218,48 @@ def test_near_threshold_samples_are_exempt_either_way(case):
     r = CMP.compare_candidates(np.append(dm, d), np.append(tt, t), np.append(cs, case["snr"][d, t]).astype(np.float32),
                                np.append(cw, case["width"][d, t]), len(dm) + 1, 1 << 20, *args)
     assert r, str(r)
+
+
+# ------------------------------------------------------------------------------------------------- decimated levels
+@pytest.fixture(scope="module")
+def dcase():
+    rng = np.random.Generator(np.random.PCG64(78))
+    x = rng.standard_normal((2, 3001)).astype(np.float32)
+    x[1, 800:860] += 1.5
+    st = O.stats(x)
+    lv = O.sweep_decimated(x, st.mean, st.sigma, float("nan"), "sqrt", 16, 4)
+    sig_all = O.sigma_table(st.sigma, float("nan"), 128, "sqrt")
+    return dict(x=x, mu=st.mean, sig=sig_all, lv=lv)
+
+
+def _lvl(c, l, g_snr=None, g_w=None):
+    L = c["lv"][l]
+    return CMP.compare_planes_level(c["x"], c["mu"], c["sig"], 16, L, L["snr"].astype(np.float32) if g_snr is None else g_snr,
+                                    L["width"].astype(np.uint16) if g_w is None else g_w)
+
+
+def test_level_planes_fp32_copy_passes(dcase):
+    for l in range(4):
+        r = _lvl(dcase, l)
+        assert r, str(r)
+
+
+def test_level_plane_errors_are_rejected(dcase):
+    L = dcase["lv"][2]
+    g = L["snr"].astype(np.float32).copy(); g[0, 10] += 2e-3
+    assert not _lvl(dcase, 2, g_snr=g)
+    w = L["width"].astype(np.uint16).copy()
+    d, i = np.argwhere((L["margin"] > 0.1) & (L["width"] > 0))[0]
+    w[d, i] = 36 if w[d, i] != 36 else 40
+    assert not _lvl(dcase, 2, g_w=w)
+    w = L["width"].astype(np.uint16).copy()
+    w[0, L["snr"].shape[1] - 1] = 36                       # a position where no width of the level fits must stay (-inf, 0)
+    assert not _lvl(dcase, 2, g_w=w)
+    g = L["snr"].astype(np.float32).copy(); g[0, L["snr"].shape[1] - 1] = 0.0
+    assert not _lvl(dcase, 2, g_snr=g)
+    w = L["width"].astype(np.uint16).copy()
+    cand = np.argwhere((L["margin"] <= CMP.TIE) & (L["width"] > 0))
+    if cand.size:                                          # inside a near-tie: a width off the level's grid is still rejected
+        d, i = cand[0]
+        w[d, i] = 38
+        assert not _lvl(dcase, 2, g_w=w)

@@ -1,0 +1,131 @@
+"""-m gpu parity of the decimated search (spd_boxcar_snr_decimated / spd_candidates_decimated, reading A20)
+against oracle O5, level by level and element by element, under the tolerances of DESIGN.md section 5."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import gen
+from oracle import compare as CMP
+from oracle import spd_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1611_09704_b200 as P
+    from paper_1611_09704_b200 import build as B
+    B.ensure_built()
+    P.lib()
+    return P
+
+
+def rng(seed):
+    return np.random.Generator(np.random.PCG64(seed))
+
+
+def _run(P, x, w0, levels, mode="sqrt", stats=None, thr=None, stride=None):
+    from gpu_util import to_dev
+    nmax = w0 << (levels - 1)
+    o = O.full_stats(x, nmax if mode != "sqrt" else 0) if stats is None else stats
+    st = P.write_stats(o.mean, o.sigma, o.sigma_nmax, o.nmax_of_sigma)
+    d = to_dev(x, stride)
+    snr, width = P.spd_boxcar_snr_decimated(d, st, w0, levels, mode)
+    lv = O.sweep_decimated(x, o.mean, o.sigma, o.sigma_nmax, mode, w0, levels)
+    sig_all = O.sigma_table(o.sigma, o.sigma_nmax, nmax, mode)
+    n_t = x.shape[1]
+    g_snr, g_w = snr.cpu().numpy(), width.cpu().numpy()
+    infos = []
+    for L in lv:
+        off, n_l = P.decimated_level_offset(n_t, L["level"]), n_t >> L["level"]
+        r = CMP.compare_planes_level(x, o.mean, sig_all, w0, L, g_snr[:, off:off + n_l], g_w[:, off:off + n_l])
+        assert r, f"level {L['level']}: {r}"
+        infos.append(r.info)
+    if thr is not None:
+        out, cnt = P.spd_candidates_decimated(snr, width, n_t, levels, thr, capacity=1 << 20)
+        rec, total = P.read_candidates(out, cnt)
+        want = 0
+        got = set(zip(rec["dm"].tolist(), rec["t"].tolist(), rec["width"].tolist()))
+        assert len(got) == total                       # one record per (level position): (dm, t, width) is unique
+        for L in lv:
+            D, off, n_l = L["D"], P.decimated_level_offset(n_t, L["level"]), n_t >> L["level"]
+            gs = g_snr[:, off:off + n_l]
+            hit = np.argwhere(gs >= np.float32(thr))    # the list is the brute filter of the GPU's own planes ...
+            want += hit.shape[0]
+            for dm, i in hit:
+                assert (int(dm), int(i) * D, int(g_w[dm, off + i])) in got
+            near = np.abs(L["snr"] - thr) <= CMP.TIE    # ... and of the oracle's, outside 1e-3 of the threshold
+            assert np.array_equal((gs >= np.float32(thr)) & ~near, (L["snr"] >= thr) & ~near)
+        assert total == want
+    return lv, infos
+
+
+@pytest.mark.parametrize("n_dm,n_t,w0,levels", [(2, 4096, 16, 1), (2, 4096, 16, 4), (3, 5003, 16, 4), (1, 2049, 32, 3),
+                                                (2, 1000, 16, 6), (1, 40, 16, 2), (2, 9001, 32, 8)])
+def test_decimated_integer_data(P, n_dm, n_t, w0, levels):
+    x = rng(500 + n_t).integers(-4, 6, size=(n_dm, n_t)).astype(np.float32)
+    _run(P, x, w0, levels, "sqrt", O.Stats(0, 0.0, 0.0, 0.0, 1.0), thr=4.0)
+
+
+@pytest.mark.parametrize("mode", ["sqrt", "linear", "anchored"])
+@pytest.mark.parametrize("mu,sigma", [(0.0, 1.0), (100.0, 20.0)])
+def test_decimated_noise_all_modes(P, mode, mu, sigma):
+    x = (mu + sigma * rng(600).standard_normal((3, 7001))).astype(np.float32)
+    x[1, 2000:2090] += 0.8 * sigma
+    lv, infos = _run(P, x, 16, 4, mode, thr=5.0, stride=7008 if mode == "linear" else None)
+    assert all(i["near_tie_rate"] < 0.08 for i in infos)
+
+
+def test_decimated_on_grid_pulse_recovers_A_sqrt_W(P):
+    n_t, A = 8192, 2.0
+    for lvl, wp in [(1, 12), (2, 16), (3, 9)]:
+        D, W, p = 1 << lvl, wp << lvl, 3200
+        x = np.zeros((1, n_t), dtype=np.float32)
+        x[0, p:p + W] = A
+        lv, _ = _run(P, x, 16, 4, "sqrt", O.Stats(0, 0.0, 0.0, 0.0, 1.0))
+        d = torch.from_numpy(x).cuda()
+        snr, width = P.spd_boxcar_snr_decimated(d, P.write_stats(0.0, 1.0), 16, 4)
+        off = P.decimated_level_offset(n_t, lvl)
+        assert int(width[0, off + p // D].item()) == W
+        assert float(snr[0, off + p // D].item()) == pytest.approx(A * math.sqrt(W), rel=3e-7)
+        assert float(snr[torch.isfinite(snr)].max().item()) == pytest.approx(A * math.sqrt(W), rel=3e-7)
+
+
+def test_decimated_level0_equals_the_exhaustive_sweep(P):
+    x = rng(601).standard_normal((4, 6000)).astype(np.float32)
+    d = torch.from_numpy(x).cuda()
+    st = P.spd_stats(d)
+    a, aw = P.spd_boxcar_snr(d, st, 16, "sqrt")
+    b, bw = P.spd_boxcar_snr_decimated(d, st, 16, 3)
+    assert torch.equal(a, b[:, :6000]) and torch.equal(aw.view(torch.int16), bw[:, :6000].view(torch.int16))
+
+
+def test_decimated_config3_rows(P):
+    """The SKA-like shape at Nmax = 128 as w0 = 16 x 4 levels on a row block of config 3, end to end with measured statistics;
+    every injected pulse of those rows is still found (sensitivity >= sqrt(0.9) of the exhaustive search)."""
+    cfg = gen.get_config(3)
+    rows = sorted(set(gen.pulse_rows(cfg)[:12]) | set(range(0, 24)))
+    x = gen.make_rows(cfg, rows)
+    d = torch.from_numpy(x).cuda()
+    st = P.spd_stats(d)
+    g = P.read_stats(st)[0]
+    o = O.stats(x)
+    assert CMP.compare_stats(float(g["mean"]), float(g["sigma"]), o)
+    lv, infos = _run(P, x, 16, 4, "sqrt", o, thr=cfg.threshold)
+    exact_snr, _, _ = O.sweep(x, o.mean, O.sigma_table(o.sigma, float("nan"), 128, "sqrt"), want_margin=False)
+    best_dec = np.max(np.stack([np.max(np.where(np.isfinite(L["snr"]), L["snr"], -np.inf), axis=1) for L in lv]), axis=0)
+    best_exact = exact_snr.max(axis=1)
+    strong = best_exact > 8.0
+    assert strong.any() and np.all(best_dec[strong] >= 0.94 * best_exact[strong])
+
+
+def test_decimated_argument_errors(P):
+    x = torch.zeros((2, 4096), device="cuda")
+    st = P.write_stats(0.0, 1.0)
+    for w0, levels in [(8, 2), (16, 0), (16, 9), (32, 8 + 1), (24, 2)]:
+        with pytest.raises(P.SpdError):
+            P.spd_boxcar_snr_decimated(x, st, w0, levels)
