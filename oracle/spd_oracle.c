@@ -18,7 +18,8 @@
  * P7 pure-noise normalisation, P8 sigma table end points, P9 candidate set = brute filter,
  * P10 (tests/test_oracle_decimated.py) for O5, decimation in time + boxcar: level 0 = O3, decimated
  * series = block sums, every level = explicit sums over the original samples, on-grid pulse = A sqrt(W),
- * off-grid sensitivity >= sqrt(0.9).
+ * off-grid sensitivity >= sqrt(0.9); P11 (tests/test_oracle_pins.py) for O3r, per-row statistics: every row equals
+ * O3 on that row alone with that row's numpy two-pass mean / std.
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -281,4 +282,35 @@ void spd_oracle_decimate2(const double *xp, int64_t n_dm, int64_t n_prev, double
     for (int64_t d = 0; d < n_dm; ++d)
         for (int64_t i = 0; i < n_l; ++i)
             xl[d * n_l + i] = xp[d * n_prev + 2 * i] + xp[d * n_prev + 2 * i + 1];
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O3r  the sweep with ONE (mu, sigma_N table) PER DM ROW  ("for the dataset": reading A3
+ * takes one estimate per call; per-row statistics, A3's alternative, is what heterogeneous data wants,
+ * SURVEY.md 8(f) f3).  Same loop as O3, with mu[d] and sig[d * nmax + (w-1)] in place of mu and sig[w-1].
+ * The per-row statistics themselves are O1 / O1b called on one row at a time (no new arithmetic).     */
+void spd_oracle_sweep_rows(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                           const double *mu, const double *sig, int nmax,
+                           double *snr, int32_t *width, double *margin)
+{
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t d = 0; d < n_dm; ++d) {
+        const float *row = x + d * row_stride;
+        const double *sg = sig + d * (int64_t)nmax;
+        for (int64_t t = 0; t < n_t; ++t) {
+            double B = 0.0, best = -INFINITY, second = -INFINITY;
+            int32_t W = 1;
+            int64_t wmax = n_t - t < (int64_t)nmax ? n_t - t : (int64_t)nmax;
+            for (int64_t w = 1; w <= wmax; ++w) {
+                B += (double)row[t + w - 1];
+                double s = (B - (double)w * mu[d]) / sg[w - 1];
+                if (s > best) { second = best; best = s; W = (int32_t)w; }
+                else if (s > second) second = s;
+            }
+            int64_t o = d * n_t + t;
+            if (snr)    snr[o] = best;
+            if (width)  width[o] = W;
+            if (margin) margin[o] = best - second;
+        }
+    }
 }

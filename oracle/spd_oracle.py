@@ -49,6 +49,8 @@ def _load():
         L.spd_oracle_sweep.argtypes = [P, i64, i64, i64, dbl, P, i32, P, P, P]
         L.spd_oracle_snr_fixed_width.argtypes = [P, i64, i64, i64, dbl, dbl, i32, P]
         L.spd_oracle_snr_at.argtypes = [P, i64, i64, dbl, P, i32, P, P, P, i64, P]
+        L.spd_oracle_sweep_rows.argtypes = [P, i64, i64, i64, P, P, i32, P, P, P]
+        L.spd_oracle_sweep_rows.restype = None
         L.spd_oracle_sweep_level.argtypes = [P, i64, i64, dbl, P, i32, i32, i32, P, P, P]
         L.spd_oracle_sweep_level.restype = None
         L.spd_oracle_decimate2.argtypes = [P, i64, i64, P]
@@ -173,6 +175,23 @@ def candidates(snr: np.ndarray, width: np.ndarray, f_T: float):
     c_snr = np.empty(cnt, dtype=np.float64); c_w = np.empty(cnt, dtype=np.int32)
     L.spd_oracle_candidates(_p(snr), _p(width), n_dm, n_t, float(f_T), cnt, _p(c_dm), _p(c_t), _p(c_snr), _p(c_w))
     return c_dm, c_t, c_snr, c_w
+
+
+def stats_rows(x: np.ndarray, nmax_for_sigma: int = 0):
+    """One Stats per DM row: O1 (and O1b) on one row at a time (reading A3's per-row alternative)."""
+    return [full_stats(x[d:d + 1], nmax_for_sigma) for d in range(x.shape[0])]
+
+
+def sweep_rows(x: np.ndarray, row_stats, nmax: int, mode):
+    """O3r: Algorithm 1 with the statistics of each row: returns (snr f64, width i32, margin f64, sig f64 [n_dm][nmax])."""
+    x, n_dm, n_t, rs = _as_x(x)
+    mu = np.ascontiguousarray([s.mean for s in row_stats], dtype=np.float64)
+    sig = np.ascontiguousarray([sigma_table(s.sigma, s.sigma_nmax, nmax, mode) for s in row_stats], dtype=np.float64)
+    snr = np.empty((n_dm, n_t), dtype=np.float64)
+    width = np.empty((n_dm, n_t), dtype=np.int32)
+    margin = np.empty((n_dm, n_t), dtype=np.float64)
+    _load().spd_oracle_sweep_rows(_p(x), n_dm, n_t, rs, _p(mu), _p(sig), int(nmax), _p(snr), _p(width), _p(margin))
+    return snr, width, margin, sig
 
 
 def decimated_levels(w0: int, levels: int):

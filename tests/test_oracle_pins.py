@@ -334,3 +334,30 @@ def test_golden_rect_pulse():
     snr, width, _ = O.sweep(x, 0.0, O.sigma_table(1.0, 0, 32, "sqrt"))
     assert np.array_equal(width[0], tab[:, 1].astype(np.int32))
     assert np.allclose(snr[0], tab[:, 2], rtol=1e-14, atol=0)
+
+
+# ------------------------------------------------------------------------------------------------- P11: per-row statistics
+def test_P11_per_row_statistics_and_sweep():
+    """O3r / stats_rows: every row's statistics are numpy's two-pass mean / std of THAT row, closed
+    forms hold per row, and the per-row sweep equals the pinned O3 run on each row alone with its own statistics."""
+    r = np.random.Generator(np.random.PCG64(1100))
+    x = np.stack([10.0 * d + (1.0 + d) * r.standard_normal(3000) for d in range(4)]).astype(np.float32)
+    x[2] = 7.0                                               # a constant row: (7, 0)
+    x[3] = np.arange(1, 3001, dtype=np.float32)              # a ramp: ((n+1)/2, sqrt((n^2-1)/12))
+    st = O.stats_rows(x, 16)
+    for d in range(4):
+        xd = x[d].astype(np.float64)
+        assert st[d].n == 3000
+        assert st[d].mean == pytest.approx(xd.mean(), rel=1e-12, abs=1e-12)
+        assert st[d].sigma == pytest.approx(xd.std(), rel=1e-12, abs=1e-12)
+        win = np.convolve(xd, np.ones(16), mode="valid")
+        assert st[d].sigma_nmax == pytest.approx(win.std(), rel=1e-10, abs=1e-9)
+    assert st[2].mean == 7.0 and st[2].sigma == 0.0
+    assert st[3].mean == pytest.approx(1500.5, rel=1e-14) and st[3].sigma == pytest.approx(math.sqrt((3000.0 ** 2 - 1) / 12), rel=1e-13)
+    rows = [0, 1, 3]                                         # sigma = 0 (row 2) is undefined input for the sweep (reading A17)
+    xs = np.ascontiguousarray(x[rows])
+    for mode in ("sqrt", "linear", "anchored"):
+        snr, width, margin, sig = O.sweep_rows(xs, [st[d] for d in rows], 16, mode)
+        for k, d in enumerate(rows):
+            s1, w1, m1 = O.sweep(x[d:d + 1], st[d].mean, O.sigma_table(st[d].sigma, st[d].sigma_nmax, 16, mode))
+            assert np.array_equal(snr[k], s1[0]) and np.array_equal(width[k], w1[0]) and np.array_equal(margin[k], m1[0])
