@@ -251,6 +251,45 @@ def extra_legs(torch, P, args, dev, step, barrier, d_x, h_x, st, ws, out, cnt, a
     return graph_ms, fused_ms, fused_kernel_ms, hits_fused, ms_e2e, hits_e2e, e2e_steps, ms_pipe, hits_pipe, pipe_steps
 
 
+def decimated_leg(torch, P, args, d_x, st, ws, n_dm, n_t, nmax, nmax_sigma, mode, thr, cap, hbm_peak):
+    """spd_stats + spd_boxcar_snr_decimated + spd_candidates_decimated (reading A20) for the same Nmax as
+    w0 = 16 x levels; an approximation of the exhaustive step (sensitivity >= sqrt(0.9)), reported beside it."""
+    if nmax < 32 or nmax % 16 or (nmax // 16) & (nmax // 16 - 1):
+        return None
+    w0, levels = 16, (nmax // 16).bit_length()
+    stride = P.decimated_level_offset(n_t, levels)
+    snr = torch.empty((n_dm, stride), dtype=torch.float32, device=d_x.device)
+    wid = torch.empty((n_dm, stride), dtype=torch.uint16, device=d_x.device)
+    dws = torch.empty(int(P.lib().spd_decimated_workspace_bytes(n_dm, n_t, w0, levels)), dtype=torch.uint8, device=d_x.device)
+    out, cnt = P.new_candidates(cap, d_x.device)
+
+    def run():
+        P.spd_stats(d_x, nmax_sigma, st, ws)
+        P.spd_boxcar_snr_decimated(d_x, st, w0, levels, mode, snr, wid, dws)
+        P.spd_candidates_decimated(snr, wid, n_t, levels, thr, out, cnt)
+    for _ in range(2):
+        run()
+    torch.cuda.synchronize()
+    steps = max(1, min(args.steps, 5))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        run()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    n = n_dm * n_t
+    frac_sum = sum(0.5 ** l for l in range(levels))
+    # bytes that must cross HBM: x read once by the statistics and once by the search, planes of every level written once and
+    # their SNR read once by the candidate selection; the decimated series are intermediates (credit: none)
+    alg_bytes = n * (4 + 4 + (4 + 2 + 4) * frac_sum)
+    return {"ms_per_step": ms, "w0": w0, "levels": levels, "hits": int(cnt.item()), "value": n / (ms * 1e-3), "unit": "samples/s per GPU",
+            "algorithmic_bytes_per_sample": alg_bytes / n, "hbm_GBps": alg_bytes / (ms * 1e-3) / 1e9,
+            "hbm_frac_of_measured": alg_bytes / (ms * 1e-3) / 1e9 / hbm_peak,
+            "note": "spd_stats + spd_boxcar_snr_decimated + spd_candidates_decimated: widths 1..16, then 18..32 step 2, 36..64 step 4, ...; "
+                    "an approximation (worst-case sensitivity sqrt(0.9) of the exhaustive search), not the headline step"}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -267,7 +306,12 @@ def run_ours(args):
     if world != args.gpus and rank == 0:
         print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; reporting n_gpus={world}", file=sys.stderr)
     torch.cuda.set_device(local)
-    if world > 1:
+    if world > 1 or args.shard == "rows":      # the sharded step all-gathers the statistics (also at world size 1)
+        if "MASTER_ADDR" not in os.environ:
+            import socket
+            with socket.socket() as sk:
+                sk.bind(("127.0.0.1", 0))
+                os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(sk.getsockname()[1]), RANK="0", WORLD_SIZE="1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
@@ -367,6 +411,9 @@ def run_ours(args):
         (graph_ms, fused_ms, fused_kernel_ms, hits_fused, ms_e2e, hits_e2e, e2e_steps, ms_pipe, hits_pipe, pipe_steps) = \
             extra_legs(torch, P, args, dev, step, barrier, d_x, h_x, st, ws, out, cnt, arena, n_dm, n_t, nmax, nmax_sigma, mode, thr, cap)
     del arena
+    dec = None
+    if extras:
+        dec = decimated_leg(torch, P, args, d_x, st, ws, n_dm, n_t, nmax, nmax_sigma, mode, thr, cap, _peaks()[0])
 
     # ---- max over ranks -------------------------------------------------------------------------------------------
     t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
@@ -429,6 +476,7 @@ def run_ours(args):
             "fused_search": {"ms_per_step": nan_to_none(fused_ms), "spd_search_fused_ms": nan_to_none(fused_kernel_ms), "hits": hits_fused,
                              "value": nan_to_none(n / (fused_ms * 1e-3)), "unit": "samples/s per GPU",
                              "note": "spd_stats + spd_search_fused (same candidate list, SNR and width planes never written); not the headline step"},
+            "decimated_search": dec,
             "hits": hits, "mean": float(stats_host["mean"]), "sigma": float(stats_host["sigma"]),
             "clocks": clocks,
             "e2e": {"value": nan_to_none(n_job / (ms_e2e * 1e-3)), "unit": "samples/s", "ms_per_step": nan_to_none(ms_e2e), "steps": e2e_steps,
@@ -446,7 +494,7 @@ def run_ours(args):
             "cpu_baseline": cpu,
         }
         print(json.dumps(res), flush=True)
-    if world > 1:
+    if dist.is_initialized():
         dist.destroy_process_group()
 
 

@@ -6,9 +6,10 @@ a compute stream, and the statistics, the hit count and the records of a finishe
 buffers.  This module is plumbing only (CUDA streams and events from PyTorch, argument marshalling); every step of
 the search runs in the kernels behind the C ABI.
 
-Chunks along TIME for the same DM trials must overlap by Nmax - 1 samples on the caller's side: the last Nmax - 1
-samples of a row see only the widths that fit (reading A9), so the next chunk starts Nmax - 1 samples
-before the end of this one and the caller drops the records of the overlap it has already seen.
+Chunks along TIME for the same DM trials must overlap by Nmax - 1 samples: the last Nmax - 1 samples of a row see only
+the widths that fit (reading A9), so the next chunk starts Nmax - 1 samples before the end of this one and the
+records of those last Nmax - 1 start samples are dropped from every chunk but the last (`time_chunks`,
+`ChunkStream.run_time_axis`): every start sample of the series is then searched exactly once with every width.
 """
 from __future__ import annotations
 
@@ -18,6 +19,21 @@ import numpy as np
 import torch
 
 from . import binding as B
+
+
+def time_chunks(n_total: int, chunk_len: int, nmax: int) -> List[Tuple[int, int, int]]:
+    """Cut a time axis of n_total samples into chunks of <= chunk_len samples that overlap by nmax - 1:
+    [(start, length, keep)]; records with local start sample t < keep belong to the chunk (all of them in the last one)."""
+    if not (1 <= nmax <= chunk_len and n_total >= 1):
+        raise ValueError("time_chunks: need 1 <= nmax <= chunk_len and n_total >= 1")
+    out, s, step = [], 0, chunk_len - (nmax - 1)
+    while True:
+        length = min(chunk_len, n_total - s)
+        last = s + length >= n_total
+        out.append((s, length, length if last else step))
+        if last:
+            return out
+        s += step
 
 
 class ChunkStream:
@@ -46,11 +62,12 @@ class ChunkStream:
         self.next_slot = 0
         self.bytes_h2d = n_dm * n_t * 4
 
-    def submit(self, h_x: torch.Tensor) -> int:
-        """Enqueue one chunk (a pinned CPU float32 [n_dm][n_t] tensor makes the copy asynchronous); returns a ticket.
-        The slot's previous result must have been collected."""
-        if h_x.is_cuda or h_x.dtype != torch.float32 or tuple(h_x.shape) != (self.n_dm, self.n_t) or not h_x.is_contiguous():
-            raise B.SpdError("h_x must be a contiguous CPU float32 [n_dm][n_t] tensor of the stream's shape")
+    def submit(self, h_x: torch.Tensor, stats: Optional[torch.Tensor] = None) -> int:
+        """Enqueue one chunk (a pinned CPU float32 [n_dm][n_t] tensor, unit time stride, makes the copy asynchronous);
+        returns a ticket.  The slot's previous result must have been collected.  `stats`: a device spd_stats_t to search
+        with (e.g. the statistics of a longer stretch of data) instead of measuring them on this chunk."""
+        if h_x.is_cuda or h_x.dtype != torch.float32 or tuple(h_x.shape) != (self.n_dm, self.n_t) or h_x.stride(1) != 1:
+            raise B.SpdError("h_x must be a CPU float32 [n_dm][n_t] tensor of the stream's shape with unit time stride")
         k = self.next_slot
         s = self.slots[k]
         if s["busy"]:
@@ -61,7 +78,10 @@ class ChunkStream:
             s["copied"].record(self.copy_stream)
         with torch.cuda.stream(self.compute_stream):
             self.compute_stream.wait_event(s["copied"])
-            B.spd_stats(s["x"], self.nsig, s["stats"], s["ws"], stream=self.compute_stream)
+            if stats is None:
+                B.spd_stats(s["x"], self.nsig, s["stats"], s["ws"], stream=self.compute_stream)
+            else:
+                s["stats"].copy_(stats, non_blocking=True)
             B.spd_search_fused(s["x"], s["stats"], self.nmax, self.mode, self.threshold, s["out"], s["cnt"], ws=s["ws"],
                                stream=self.compute_stream)
             s["h_cnt"].copy_(s["cnt"], non_blocking=True)
@@ -83,6 +103,34 @@ class ChunkStream:
         got = min(total, self.capacity)
         rec = s["h_out"][:got].numpy().view(B.CAND_DTYPE).reshape(-1)
         return rec, total, s["h_stats"].numpy().view(B.STATS_DTYPE)
+
+    def run_time_axis(self, h_series: torch.Tensor, stats: Optional[torch.Tensor] = None) -> Tuple[np.ndarray, int]:
+        """Search a long series [n_dm][T] (pinned CPU tensor) as consecutive chunks of the stream's n_t samples that
+        overlap by nmax - 1; returns (records with t in samples of the SERIES, number of records).  The last chunk must
+        have the stream's length too: T = n_t + k (n_t - nmax + 1)."""
+        T = h_series.shape[1]
+        plan = time_chunks(T, self.n_t, self.nmax)
+        if any(length != self.n_t for _, length, _ in plan):
+            raise B.SpdError("run_time_axis: the series length must be n_t + k (n_t - nmax + 1)")
+        recs: List[np.ndarray] = []
+        tickets: List[Tuple[int, int, int]] = []
+
+        def collect():
+            tk, start, keep = tickets.pop(0)
+            rec, total, _ = self.result(tk)
+            if total > self.capacity:
+                raise B.SpdError("run_time_axis: candidate buffer overflow")
+            r = rec[rec["t"] < keep].copy()
+            r["t"] += np.uint32(start)
+            recs.append(r)
+        for start, length, keep in plan:
+            if len(tickets) == len(self.slots):
+                collect()
+            tickets.append((self.submit(h_series[:, start:start + length], stats), start, keep))
+        while tickets:
+            collect()
+        out = np.concatenate(recs) if recs else np.zeros(0, dtype=B.CAND_DTYPE)
+        return out, int(out.size)
 
     def run(self, chunks: List[torch.Tensor]) -> List[Tuple[np.ndarray, int]]:
         """Convenience: push a list of chunks through the pipeline in order; returns copies of (records, count)."""

@@ -42,6 +42,51 @@ def test_chunk_stream_equals_search_host(P, mode, nmax):
     assert len(set(counts)) > 1 and min(counts) > 0        # the chunks differ, and every one has detections
 
 
+@pytest.mark.parametrize("mode,nmax", [("sqrt", 32), ("sqrt", 100), ("anchored", 64)])
+def test_time_axis_chunks_with_overlap_equal_the_oracle_on_the_whole_series(P, mode, nmax):
+    """Consecutive chunks along TIME overlap by Nmax - 1 (stream.time_chunks); with the statistics of the whole series the
+    union of their records must be the ORACLE's candidate list of the concatenated series: every start sample searched
+    exactly once, with every width (reading A9)."""
+    from oracle import spd_oracle as O
+    from oracle import compare as CMP
+    from paper_1611_09704_b200.stream import ChunkStream, time_chunks
+    n_dm, n_t, k = 3, 4096, 4
+    T = n_t + k * (n_t - nmax + 1)
+    rng = np.random.Generator(np.random.PCG64(900 + nmax))
+    x = (2.0 + 1.5 * rng.standard_normal((n_dm, T))).astype(np.float32)
+    for c in range(1, k + 1):                              # pulses straddling every chunk boundary, and one at the very end
+        b = c * (n_t - nmax + 1)
+        x[c % n_dm, b - nmax // 2:b + nmax // 3] += 1.5
+    x[0, T - 20:] += 4.0
+    thr = 5.0
+    o = O.search(x, nmax, mode, thr)
+    st = o["stats"]
+    assert [p[:2] for p in time_chunks(T, n_t, nmax)][:2] == [(0, n_t), (n_t - nmax + 1, n_t)]
+    d_st = P.write_stats(st.mean, st.sigma, st.sigma_nmax, st.nmax_of_sigma)
+    cs = ChunkStream(n_dm, n_t, nmax, mode, thr, capacity=1 << 16, depth=2)
+    rec, total = cs.run_time_axis(torch.from_numpy(x).pin_memory(), d_st)
+    r = CMP.compare_candidates(rec["dm"], rec["t"], rec["snr"], rec["width"], total, 1 << 16, o["snr"], o["width"], o["margin"], thr,
+                               x, st.mean, o["sig"])
+    assert r, str(r)
+    assert r.info["oracle_hits"] > 50 and (rec["t"] >= T - 20).any()
+
+
+def test_chunk_stream_records_against_the_oracle(P):
+    """ChunkStream output chunk by chunk against oracle.search (not against another CUDA call)."""
+    from oracle import spd_oracle as O
+    from oracle import compare as CMP
+    from paper_1611_09704_b200.stream import ChunkStream
+    base = gen.get_config(1)
+    chunks_np = [gen.make_array(dataclasses.replace(base, cid=base.cid + 100 * k)) for k in range(3)]
+    cs = ChunkStream(base.n_dm, base.n_t, 32, "sqrt", base.threshold, capacity=4096, depth=2)
+    got = cs.run([torch.from_numpy(c).pin_memory() for c in chunks_np])
+    for c, (rec, total) in zip(chunks_np, got):
+        o = O.search(c, 32, "sqrt", base.threshold)
+        r = CMP.compare_candidates(rec["dm"], rec["t"], rec["snr"], rec["width"], total, 4096, o["snr"], o["width"], o["margin"],
+                                   base.threshold, c, o["stats"].mean, o["sig"])
+        assert r, str(r)
+
+
 def test_chunk_stream_refuses_to_overrun_its_slots(P):
     from paper_1611_09704_b200.stream import ChunkStream
     cs = ChunkStream(4, 2048, 8, "sqrt", 5.0, capacity=64, depth=1)
