@@ -113,6 +113,23 @@ spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t
                             spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,
                             void *d_ws, size_t ws_bytes, void *stream);
 
+/* Per-DM-row statistics ("for the dataset": reading A3 takes one estimate per call over everything passed
+ * in; one estimate per DM trial is the alternative heterogeneous data wants).
+ * spd_stats_rows writes d_stats_rows[n_dm], one spd_stats_t per row (same kernels and precision as spd_stats, one row per
+ * grid slice); spd_boxcar_snr_rows / spd_search_fused_rows are spd_boxcar_snr / spd_search_fused with mu, sigma (and
+ * sigma_nmax) of row d taken from d_stats_rows[d].  d_ws: >= spd_workspace_bytes_rows() bytes, 16-byte aligned (block
+ * partials of the statistics; one r_w table per row in the eq. 5 modes).  A row with sigma = 0 is undefined input. */
+size_t spd_workspace_bytes_rows(int64_t n_dm, int64_t n_t, int nmax);
+spd_status spd_stats_rows(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
+                          spd_stats_t *d_stats_rows, void *d_ws, size_t ws_bytes, void *stream);
+spd_status spd_boxcar_snr_rows(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                               const spd_stats_t *d_stats_rows, int nmax, spd_sigma_mode mode,
+                               float *d_snr, uint16_t *d_width, void *d_ws, size_t ws_bytes, void *stream);
+spd_status spd_search_fused_rows(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                                 const spd_stats_t *d_stats_rows, int nmax, spd_sigma_mode mode, float threshold,
+                                 spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,
+                                 void *d_ws, size_t ws_bytes, void *stream);
+
 /* Decimation in time + boxcar for wide filters (section 3: "a combination of boxcar filtering with the
  * decimation in time of the input data"; the paper names the route, the algorithm is reading A20 of DESIGN.md).
  * An APPROXIMATION of spd_boxcar_snr with nmax = w0 * 2^(levels-1): the width grid gets coarser with width

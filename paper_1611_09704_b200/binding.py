@@ -52,12 +52,17 @@ def lib() -> C.CDLL:
         L.spd_search_fused.argtypes = [vp, i64, i64, i64, vp, i32, i32, f32, vp, u64, vp, vp, sz, vp]
         L.spd_search_host_arena_bytes.argtypes = [i64, i64, i32, u64]; L.spd_search_host_arena_bytes.restype = sz
         L.spd_search_host.argtypes = [vp, i64, i64, i32, i32, f32, vp, u64, vp, vp, vp, sz, vp]
+        L.spd_workspace_bytes_rows.argtypes = [i64, i64, i32]; L.spd_workspace_bytes_rows.restype = sz
+        L.spd_stats_rows.argtypes = [vp, i64, i64, i64, i32, vp, vp, sz, vp]
+        L.spd_boxcar_snr_rows.argtypes = [vp, i64, i64, i64, vp, i32, i32, vp, vp, vp, sz, vp]
+        L.spd_search_fused_rows.argtypes = [vp, i64, i64, i64, vp, i32, i32, f32, vp, u64, vp, vp, sz, vp]
         L.spd_decimated_level_offset.argtypes = [i64, i32]; L.spd_decimated_level_offset.restype = i64
         L.spd_decimated_workspace_bytes.argtypes = [i64, i64, i32, i32]; L.spd_decimated_workspace_bytes.restype = sz
         L.spd_boxcar_snr_decimated.argtypes = [vp, i64, i64, i64, vp, i32, i32, i32, vp, vp, i64, vp, sz, vp]
         L.spd_candidates_decimated.argtypes = [vp, vp, i64, i64, i64, i32, f32, vp, u64, vp, vp]
         for f in ("spd_stats", "spd_stats_merge", "spd_boxcar_snr", "spd_candidates", "spd_search_fused", "spd_search_host",
-                  "spd_boxcar_snr_decimated", "spd_candidates_decimated"):
+                  "spd_boxcar_snr_decimated", "spd_candidates_decimated", "spd_stats_rows", "spd_boxcar_snr_rows",
+                  "spd_search_fused_rows"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -163,6 +168,52 @@ def spd_search_fused(x: torch.Tensor, stats: torch.Tensor, nmax: int, mode, thre
     _check(lib().spd_search_fused(x.data_ptr(), n_dm, n_t, rs, stats.data_ptr(), int(nmax), _MODES[mode], float(threshold),
                                   out.data_ptr(), out.shape[0], count.data_ptr(), ws.data_ptr(), ws.numel(),
                                   _stream(stream)), "spd_search_fused")
+    return out, count
+
+
+def new_workspace_rows(n_dm: int, n_t: int, nmax: int, device="cuda") -> torch.Tensor:
+    return torch.empty(max(256, int(lib().spd_workspace_bytes_rows(n_dm, n_t, max(nmax, 1)))), dtype=torch.uint8, device=device)
+
+
+def spd_stats_rows(x: torch.Tensor, nmax_for_sigma: int = 0, stats: Optional[torch.Tensor] = None,
+                   ws: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """One spd_stats_t per DM row: uint8[n_dm * 80] on the device (read_stats gives the structured array)."""
+    n_dm, n_t, rs = _plane(x, torch.float32, "x")
+    stats = new_stats(x.device, n_dm) if stats is None else stats
+    ws = new_workspace_rows(n_dm, n_t, nmax_for_sigma, x.device) if ws is None else ws
+    _check(lib().spd_stats_rows(x.data_ptr(), n_dm, n_t, rs, int(nmax_for_sigma), stats.data_ptr(), ws.data_ptr(), ws.numel(),
+                                _stream(stream)), "spd_stats_rows")
+    return stats
+
+
+def spd_boxcar_snr_rows(x: torch.Tensor, stats_rows: torch.Tensor, nmax: int, mode="sqrt",
+                        snr: Optional[torch.Tensor] = None, width: Optional[torch.Tensor] = None,
+                        ws: Optional[torch.Tensor] = None, stream=None):
+    n_dm, n_t, rs = _plane(x, torch.float32, "x")
+    if stats_rows.numel() != n_dm * STATS_BYTES:
+        raise SpdError("stats_rows must hold one spd_stats_t per DM row")
+    if snr is None:
+        snr = torch.empty_strided((n_dm, n_t), (rs, 1), dtype=torch.float32, device=x.device)
+    if width is None:
+        width = torch.empty_strided((n_dm, n_t), (rs, 1), dtype=torch.uint16, device=x.device)
+    ws = new_workspace_rows(n_dm, n_t, nmax, x.device) if ws is None else ws
+    _check(lib().spd_boxcar_snr_rows(x.data_ptr(), n_dm, n_t, rs, stats_rows.data_ptr(), int(nmax), _MODES[mode], snr.data_ptr(),
+                                     width.data_ptr(), ws.data_ptr(), ws.numel(), _stream(stream)), "spd_boxcar_snr_rows")
+    return snr, width
+
+
+def spd_search_fused_rows(x: torch.Tensor, stats_rows: torch.Tensor, nmax: int, mode, threshold: float,
+                          out: Optional[torch.Tensor] = None, count: Optional[torch.Tensor] = None,
+                          capacity: int = 1 << 20, ws: Optional[torch.Tensor] = None, stream=None):
+    n_dm, n_t, rs = _plane(x, torch.float32, "x")
+    if stats_rows.numel() != n_dm * STATS_BYTES:
+        raise SpdError("stats_rows must hold one spd_stats_t per DM row")
+    if out is None or count is None:
+        out, count = new_candidates(capacity, x.device)
+    ws = new_workspace_rows(n_dm, n_t, nmax, x.device) if ws is None else ws
+    _check(lib().spd_search_fused_rows(x.data_ptr(), n_dm, n_t, rs, stats_rows.data_ptr(), int(nmax), _MODES[mode], float(threshold),
+                                       out.data_ptr(), out.shape[0], count.data_ptr(), ws.data_ptr(), ws.numel(),
+                                       _stream(stream)), "spd_search_fused_rows")
     return out, count
 
 

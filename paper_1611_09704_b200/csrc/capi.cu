@@ -106,6 +106,65 @@ spd_status spd_search_fused(const float *d_x, int64_t n_dm, int64_t n_t, int64_t
     return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
 }
 
+// ---- one (mu, sigma) per DM row (reading A3's alternative) ---------------------------------
+size_t spd_workspace_bytes_rows(int64_t n_dm, int64_t n_t, int nmax)
+{
+    if (n_dm < 1 || n_t < 1 || nmax < 0 || nmax > NMAX_API_LIMIT) return 0;
+    const size_t tab = (size_t)n_dm * sweep_table_bytes(nmax > 0 ? nmax : 1);
+    const size_t st = stats_rows_ws_bytes(n_dm);
+    return align_up(st > tab ? st : tab, 256);
+}
+
+spd_status spd_stats_rows(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
+                          spd_stats_t *d_stats_rows, void *d_ws, size_t ws_bytes, void *stream)
+{
+    if (!d_x || !d_stats_rows || !d_ws || !shape_ok(n_dm, n_t, row_stride)) return SPD_ERR_INVALID_ARG;
+    if (nmax_for_sigma < 0 || (nmax_for_sigma > 0 && !nmax_ok(nmax_for_sigma, n_t))) return SPD_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_ws) & 15) != 0) return SPD_ERR_INVALID_ARG;
+    if (ws_bytes < stats_rows_ws_bytes(n_dm)) return SPD_ERR_WORKSPACE;
+    cudaError_t e = launch_stats_rows(d_x, n_dm, n_t, row_stride, nmax_for_sigma, d_stats_rows, d_ws, (cudaStream_t)stream);
+    return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
+}
+
+spd_status spd_boxcar_snr_rows(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                               const spd_stats_t *d_stats_rows, int nmax, spd_sigma_mode mode,
+                               float *d_snr, uint16_t *d_width, void *d_ws, size_t ws_bytes, void *stream)
+{
+    if (!d_x || !d_stats_rows || !d_snr || !d_ws || !shape_ok(n_dm, n_t, row_stride) || !nmax_ok(nmax, n_t))
+        return SPD_ERR_INVALID_ARG;
+    if ((int)mode < 0 || (int)mode > 2 || (reinterpret_cast<uintptr_t>(d_ws) & 15) != 0) return SPD_ERR_INVALID_ARG;
+    const bool rc = sweep_uses_constant_table(nmax, (int)mode);
+    if (!rc && ws_bytes < (size_t)n_dm * sweep_table_bytes(nmax)) return SPD_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    float *table = reinterpret_cast<float *>(d_ws);
+    cudaError_t e = rc ? cudaSuccess : launch_sigma_table(d_stats_rows, nmax, (int)mode, table, s, 1, 0, n_dm);
+    if (e != cudaSuccess) return SPD_ERR_CUDA;
+    e = launch_sweep(d_x, n_dm, n_t, row_stride, d_stats_rows, table, nmax, rc, d_snr, d_width, false, 0.0f, nullptr, 0, nullptr, s, 1);
+    return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
+}
+
+spd_status spd_search_fused_rows(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                                 const spd_stats_t *d_stats_rows, int nmax, spd_sigma_mode mode, float threshold,
+                                 spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,
+                                 void *d_ws, size_t ws_bytes, void *stream)
+{
+    if (!d_x || !d_stats_rows || !d_count || (!d_out && capacity > 0) || !d_ws || !shape_ok(n_dm, n_t, row_stride) ||
+        !nmax_ok(nmax, n_t))
+        return SPD_ERR_INVALID_ARG;
+    if ((int)mode < 0 || (int)mode > 2 || threshold != threshold || (reinterpret_cast<uintptr_t>(d_ws) & 15) != 0)
+        return SPD_ERR_INVALID_ARG;
+    const bool rc = sweep_uses_constant_table(nmax, (int)mode);
+    if (!rc && ws_bytes < (size_t)n_dm * sweep_table_bytes(nmax)) return SPD_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    float *table = reinterpret_cast<float *>(d_ws);
+    if (cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s) != cudaSuccess) return SPD_ERR_CUDA;
+    cudaError_t e = rc ? cudaSuccess : launch_sigma_table(d_stats_rows, nmax, (int)mode, table, s, 1, 0, n_dm);
+    if (e != cudaSuccess) return SPD_ERR_CUDA;
+    e = launch_sweep(d_x, n_dm, n_t, row_stride, d_stats_rows, table, nmax, rc, nullptr, nullptr, true, threshold, d_out,
+                     capacity, d_count, s, 1);
+    return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
+}
+
 // ---- decimation in time + boxcar (reading A20) ----------------------------------------------------
 namespace {
 inline bool dec_ok(int w0, int levels, int64_t n_t) { return (w0 == 16 || w0 == 32) && levels >= 1 && levels <= 8 && (int64_t)w0 <= n_t && (w0 << (levels - 1)) <= NMAX_API_LIMIT; }

@@ -41,9 +41,12 @@ __host__ __device__ inline int round_up(int a, int b) { return (a + b - 1) / b *
 // ---- launchers (defined in the .cu files) ---------------------------------------------------------------
 cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
                          spd_stats_t *d_stats, void *d_ws, cudaStream_t s);
+cudaError_t launch_stats_rows(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
+                              spd_stats_t *d_stats_rows, void *d_ws, cudaStream_t s);
+size_t stats_rows_ws_bytes(int64_t n_dm);
 cudaError_t launch_stats_merge(const spd_stats_t *parts, int count, spd_stats_t *out, cudaStream_t s);
 cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, float *d_table, cudaStream_t s,
-                               int wscale = 1, int nmax_total = 0);
+                               int wscale = 1, int nmax_total = 0, int64_t rows = 1);
 cudaError_t launch_decimate2(const float *src, int64_t n_dm, int64_t n_l, int64_t src_stride, float *dst, int64_t dst_stride, cudaStream_t s);
 cudaError_t launch_level_stats(const spd_stats_t *st, int D, spd_stats_t *out, cudaStream_t s);
 cudaError_t launch_sweep_level(const float *xl, int64_t n_dm, int64_t n_l, int64_t xl_stride, const spd_stats_t *d_stats_level,
@@ -53,7 +56,7 @@ bool sweep_uses_constant_table(int nmax, int mode);      // eq. 4 with nmax a mu
 cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
                          const float *d_table, int nmax, bool rc, float *snr, uint16_t *width,
                          bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
-                         unsigned long long *d_count, cudaStream_t s);
+                         unsigned long long *d_count, cudaStream_t s, int stats_stride = 0);
 cudaError_t launch_candidates(const float *snr, const uint16_t *width, int64_t n_dm, int64_t n_t, int64_t row_stride,
                               float threshold, spd_candidate_t *out, unsigned long long capacity,
                               unsigned long long *d_count, cudaStream_t s, bool zero_count = true, uint32_t t_scale = 1);

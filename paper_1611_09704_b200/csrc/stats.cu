@@ -135,6 +135,9 @@ __device__ __forceinline__ void write_partial(Tri *warp_acc, const Tri &acc, dou
 __global__ void __launch_bounds__(ST_THREADS)
 stats_partial(const float *__restrict__ x, int64_t n_rows, int64_t n_t, int64_t row_stride, Tri *__restrict__ partials)
 {
+    // per-row statistics (spd_stats_rows): gridDim.y = rows, every y-slice is an independent one-row problem
+    x += (int64_t)blockIdx.y * row_stride;
+    partials += (size_t)blockIdx.y * gridDim.x;
     __shared__ Tri warp_acc[ST_THREADS / 32];
     __shared__ float red[2 * ST_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31;
@@ -215,6 +218,9 @@ __global__ void __launch_bounds__(ST_THREADS, 3)
 stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax,
                   Tri *__restrict__ part_x, Tri *__restrict__ part_b)
 {
+    x += (int64_t)blockIdx.y * row_stride;                     // per-row statistics: gridDim.y = rows (n_dm = 1 per slice)
+    part_x += (size_t)blockIdx.y * gridDim.x;
+    part_b += (size_t)blockIdx.y * gridDim.x;
     extern __shared__ __align__(16) unsigned char st_smem[];
     __shared__ Tri warp_acc[ST_THREADS / 32];
     __shared__ float red[2 * ST_THREADS / 32];
@@ -390,6 +396,20 @@ stats_finalize(const Tri *__restrict__ part_x, int count_x, const Tri *__restric
     if (threadIdx.x == 0) fill_stats(out, a, b, nmax_of_sigma);
 }
 
+// per-row variant of kernel 2: CTA r folds the partials of row r (a handful) in index order
+__global__ void stats_finalize_rows(const Tri *__restrict__ part_x, const Tri *__restrict__ part_b, int per_row, int nmax_of_sigma,
+                                    spd_stats_t *__restrict__ out)
+{
+    if (threadIdx.x != 0) return;
+    const size_t r = blockIdx.x;
+    Tri a = {0.0, 0.0, 0.0}, b = {0.0, 0.0, 0.0};
+    for (int i = 0; i < per_row; ++i) {
+        tri_merge(a, part_x[r * per_row + i]);
+        if (nmax_of_sigma > 0) tri_merge(b, part_b[r * per_row + i]);
+    }
+    fill_stats(out + r, a, b, nmax_of_sigma);
+}
+
 // eq. 2 over whole results (the exchange step of a DM-row-sharded run), folded in index order.  Parts with no samples
 // (a rank that holds no rows contributes an all-zero struct) are skipped, also in the nmax_of_sigma consistency check.
 __global__ void stats_merge_kernel(const spd_stats_t *__restrict__ parts, int count, spd_stats_t *__restrict__ out)
@@ -407,6 +427,21 @@ __global__ void stats_merge_kernel(const spd_stats_t *__restrict__ parts, int co
     fill_stats(out, a, b, nm < 0 ? 0 : nm);
 }
 
+// per device: the dynamic shared-memory limit of stats_partial_win, set once to the largest tile (nmax = 4096)
+static cudaError_t stats_win_limit()
+{
+    static bool limit_set[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !limit_set[dev]) {
+        e = cudaFuncSetAttribute(stats_partial_win, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * st_pad(ST_CHUNK + 4096 + 2 * ST_RUN) * sizeof(float)));
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) limit_set[dev] = true;
+    }
+    return cudaSuccess;
+}
+
 cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
                          spd_stats_t *d_stats, void *d_ws, cudaStream_t s)
 {
@@ -417,15 +452,8 @@ cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
         gx = gb = (int)(tiles < ST_GRID ? tiles : ST_GRID);
         const int span4 = (ST_CHUNK + nmax_for_sigma - 1 + 3) & ~3;
         const size_t smem = (size_t)(st_pad(span4 + ST_RUN) + st_pad(span4 + 2 * ST_RUN)) * sizeof(float);
-        static bool limit_set[64] = {};                        // per device: the kernel's dynamic shared-memory limit, set once to the largest tile (nmax = 4096)
-        int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
+        cudaError_t e = stats_win_limit();
         if (e != cudaSuccess) return e;
-        if (dev < 0 || dev >= 64 || !limit_set[dev]) {
-            e = cudaFuncSetAttribute(stats_partial_win, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * st_pad(ST_CHUNK + 4096 + 2 * ST_RUN) * sizeof(float)));
-            if (e != cudaSuccess) return e;
-            if (dev >= 0 && dev < 64) limit_set[dev] = true;
-        }
         stats_partial_win<<<gx, ST_THREADS, smem, s>>>(x, n_dm, n_t, row_stride, nmax_for_sigma, px, pb);
     } else {
         int64_t rows = n_dm, cols = n_t, stride = row_stride;
@@ -435,6 +463,35 @@ cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
         stats_partial<<<gx, ST_THREADS, 0, s>>>(x, rows, cols, stride, px);
     }
     stats_finalize<<<1, ST_THREADS, 0, s>>>(px, gx, pb, gb, nmax_for_sigma, d_stats);
+    return cudaGetLastError();
+}
+
+// ---- one (mu, sigma, sigma_nmax) per DM row (reading A3's alternative) ----
+constexpr int ST_ROW_CTAS = 8;                                  // CTAs that share one row
+size_t stats_rows_ws_bytes(int64_t n_dm) { return (size_t)n_dm * ST_ROW_CTAS * 2 * sizeof(Tri); }
+
+cudaError_t launch_stats_rows(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
+                              spd_stats_t *d_stats_rows, void *d_ws, cudaStream_t s)
+{
+    const int64_t cpr = (n_t + ST_CHUNK - 1) / ST_CHUNK;
+    const int gx = (int)(cpr < ST_ROW_CTAS ? cpr : ST_ROW_CTAS);
+    Tri *px = reinterpret_cast<Tri *>(d_ws), *pb = px + (size_t)n_dm * gx;
+    cudaError_t e;
+    size_t smem = 0;
+    if (nmax_for_sigma > 0) {
+        if ((e = stats_win_limit()) != cudaSuccess) return e;
+        const int span4 = (ST_CHUNK + nmax_for_sigma - 1 + 3) & ~3;
+        smem = (size_t)(st_pad(span4 + ST_RUN) + st_pad(span4 + 2 * ST_RUN)) * sizeof(float);
+    }
+    for (int64_t r0 = 0; r0 < n_dm; r0 += 65535) {               // grid.y limit
+        const unsigned ny = (unsigned)(n_dm - r0 < 65535 ? n_dm - r0 : 65535);
+        const float *xr = x + r0 * row_stride;
+        if (nmax_for_sigma > 0)
+            stats_partial_win<<<dim3(gx, ny), ST_THREADS, smem, s>>>(xr, 1, n_t, row_stride, nmax_for_sigma, px + (size_t)r0 * gx, pb + (size_t)r0 * gx);
+        else
+            stats_partial<<<dim3(gx, ny), ST_THREADS, 0, s>>>(xr, 1, n_t, row_stride, px + (size_t)r0 * gx);
+    }
+    stats_finalize_rows<<<(unsigned)n_dm, 32, 0, s>>>(px, pb, gx, nmax_for_sigma, d_stats_rows);
     return cudaGetLastError();
 }
 

@@ -114,6 +114,8 @@ __device__ __forceinline__ void cp_async_commit_wait_all()
 __global__ void sigma_table_kernel(const spd_stats_t *__restrict__ st, int nmax, int mode, float *__restrict__ table,
                                    int wscale, int nmax_total)
 {
+    st += blockIdx.y;                               // per-row statistics: one table per row (grid.y = rows, else 1)
+    table += (size_t)blockIdx.y * sw_rt_len(nmax);
     const double sigma = st->sigma, snm = st->sigma_nmax;
     const bool bad = (mode != SPD_SIGMA_SQRT) && (st->nmax_of_sigma != nmax_total);
     for (int w = 1 + blockIdx.x * blockDim.x + threadIdx.x; w <= sw_rt_len(nmax); w += gridDim.x * blockDim.x) {
@@ -130,10 +132,15 @@ __global__ void sigma_table_kernel(const spd_stats_t *__restrict__ st, int nmax,
     }
 }
 
-cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, float *d_table, cudaStream_t s, int wscale, int nmax_total)
+cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, float *d_table, cudaStream_t s, int wscale, int nmax_total,
+                               int64_t rows)
 {
     int n = sw_rt_len(nmax);
-    sigma_table_kernel<<<(n + 255) / 256, 256, 0, s>>>(d_stats, nmax, mode, d_table, wscale, nmax_total > 0 ? nmax_total : nmax);
+    for (int64_t r0 = 0; r0 < rows; r0 += 65535) {               // grid.y limit
+        const unsigned ny = (unsigned)(rows - r0 < 65535 ? rows - r0 : 65535);
+        sigma_table_kernel<<<dim3((n + 255) / 256, ny), 256, 0, s>>>(d_stats + r0, nmax, mode, d_table + (size_t)r0 * n, wscale,
+                                                                      nmax_total > 0 ? nmax_total : nmax);
+    }
     return cudaGetLastError();
 }
 
@@ -273,7 +280,8 @@ struct TileStager {
 // What every sweep kernel needs from the statistics: y = ((x - mu_hi) - mu_lo) [* 1/sigma when RC]
 struct Norm {
     float2 mu_hi2, mu_lo2, rs2;
-    __device__ __forceinline__ Norm(const spd_stats_t *st)
+    __device__ __forceinline__ Norm(const spd_stats_t *st) { load(st); }
+    __device__ __forceinline__ void load(const spd_stats_t *st)
     {
         const double mu = st->mean;
         const float mu_hi = (float)mu, mu_lo = (float)(mu - (double)mu_hi), rs = (float)(1.0 / st->sigma);
@@ -409,7 +417,8 @@ template <int SW_THREADS, bool RC>
 __global__ void __launch_bounds__(SW_THREADS, 512 / SW_THREADS)
 boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                  const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
-                 float *__restrict__ snr, uint16_t *__restrict__ width)
+                 float *__restrict__ snr, uint16_t *__restrict__ width,
+                 int stats_stride /* 0: one spd_stats_t (and table) for all rows; 1: one per DM row */)
 {
     constexpr int SW_SUB = SW_THREADS * SW_R, SW_TILE = 2 * SW_SUB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -428,11 +437,12 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
     const int LRAW = SW_TILE + H;                 // raw floats per tile: x[T0 .. T0 + TILE + H)
     const int LZ = SW_SUB + H;                    // interleaved positions (a multiple of 8)
     const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
-    const Norm norm(st);
+    Norm norm(st);
     const float NINF = __int_as_float(0xff800000);
     const int mask7 = opaque_reg(~7);
+    const bool row_tables = !RC && stats_stride != 0;
 
-    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = RC ? c_isqrt.v[w] : __ldg(table + w);
+    if (!row_tables) for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = RC ? c_isqrt.v[w] : __ldg(table + w);
 
     int64_t tile = blockIdx.x;
     TilePos pos(blockIdx.x, tiles_per_row);
@@ -445,6 +455,13 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
         const int64_t row = pos.row;
         const int64_t T0 = (int64_t)pos.tr * SW_TILE;
         pos = pos.next(gridDim.x, tiles_per_row);                                  // the tile after this one
+        if (stats_stride) {                        // per-row statistics: this row's mu, sigma (and r_w table)
+            norm.load(st + row);
+            if (row_tables) {
+                __syncthreads();                   // the width search of the previous tile has read rtf
+                for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + row * sw_rt_len(nmax) + w);
+            }
+        }
         stg.wait();
         __syncthreads();                           // raw tile landed; everyone is done with the previous Z / E
 
@@ -604,7 +621,7 @@ __global__ void __launch_bounds__(SW_THREADS, 512 / SW_THREADS)
 boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                     const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
                     float threshold, spd_candidate_t *__restrict__ cand, unsigned long long capacity,
-                    unsigned long long *__restrict__ count)
+                    unsigned long long *__restrict__ count, int stats_stride)
 {
     constexpr int SW_SUB = SW_THREADS * SW_R, SW_TILE = 2 * SW_SUB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -618,10 +635,11 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
     const int H = sw_halo(nmax);
     const int LRAW = SW_TILE + H, LZ = SW_SUB + H;
     const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
-    const Norm norm(st);
+    Norm norm(st);
     const float NINF = __int_as_float(0xff800000);
+    const bool row_tables = !RC && stats_stride != 0;
 
-    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = RC ? c_isqrt.v[w] : __ldg(table + w);
+    if (!row_tables) for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = RC ? c_isqrt.v[w] : __ldg(table + w);
     // a NaN reciprocal table (LINEAR mode fed stats of another Nmax): NaN >= threshold is false everywhere, which would
     // read as "no detections"; report the misuse as count = ~0 instead (spd.h)
     if (!RC && blockIdx.x == 0 && tid == 0) { const float r0 = __ldg(table); if (r0 != r0) *count = ~0ULL; }
@@ -637,6 +655,13 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
         const int64_t row = pos.row;
         const int64_t T0 = (int64_t)pos.tr * SW_TILE;
         pos = pos.next(gridDim.x, tiles_per_row);                                  // the tile after this one
+        if (stats_stride) {
+            norm.load(st + row);
+            if (row_tables) {
+                __syncthreads();                   // the replays of the previous tile have read rtf
+                for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + row * sw_rt_len(nmax) + w);
+            }
+        }
         stg.wait();
         __syncthreads();                           // raw tile landed; everyone is done with the previous Z
 
@@ -662,7 +687,12 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
         {
             const float2 *zp = Z + 9 * (tid + 1);
             const float *rp = rtf;
-            for (int kb = 0; kb < nblk; ++kb, zp += 9, rp += 8) sweep8<RC>(B, W, best, best, zp, rp, 8 * kb);
+            int kb = 0;
+            for (; kb + 2 <= nblk; kb += 2, zp += 18, rp += 16) {
+                sweep8<RC>(B, W, best, best, zp, rp, 8 * kb);
+                sweep8<RC>(B, W, best, best, zp + 9, rp + 8, 8 * kb + 8);
+            }
+            if (kb < nblk) sweep8<RC>(B, W, best, best, zp, rp, 8 * kb);
         }
 
         // ---- threshold; hits replay their own running sums to get the width ------------------------------------------
@@ -731,7 +761,8 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
                         const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
                         float *__restrict__ snr, uint16_t *__restrict__ width,
                         int wmin /* widths <= wmin are summed but not evaluated (0 or a multiple of 8) */,
-                        int wscale /* reported width = w * wscale */, int64_t out_stride /* row stride of the planes */)
+                        int wscale /* reported width = w * wscale */, int64_t out_stride /* row stride of the planes */,
+                        int stats_stride)
 {
     constexpr int SW_SUB = SW_THREADS * SW_R, SW_TILE = 2 * SW_SUB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -745,11 +776,12 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
     const int H = sw_halo(nmax);
     const int LRAW = SW_TILE + H, LZ = SW_SUB + H;
     const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
-    const Norm norm(st);
+    Norm norm(st);
     const float NINF = __int_as_float(0xff800000);
     const int mask31 = opaque_reg(~31);
+    const bool row_tables = !RC && stats_stride != 0;
 
-    if (!RC) for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
+    if (!RC && !row_tables) for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
 
     int64_t tile = blockIdx.x;
     TilePos pos(blockIdx.x, tiles_per_row);
@@ -762,6 +794,13 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
         const int64_t row = pos.row;
         const int64_t T0 = (int64_t)pos.tr * SW_TILE;
         pos = pos.next(gridDim.x, tiles_per_row);                                  // the tile after this one
+        if (stats_stride) {
+            norm.load(st + row);
+            if (row_tables) {
+                __syncthreads();                   // the width loop of the previous tile has read rtf
+                for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + row * sw_rt_len(nmax) + w);
+            }
+        }
         stg.wait();
         __syncthreads();                           // raw tile landed; everyone is done with the previous Z
 
@@ -864,7 +903,7 @@ template <int NT, bool RC>
 static cudaError_t launch_sweep_nt(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
                                    const float *d_table, int nmax, float *snr, uint16_t *width,
                                    bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
-                                   unsigned long long *d_count, cudaStream_t s)
+                                   unsigned long long *d_count, cudaStream_t s, int stats_stride)
 {
     constexpr int TILE = 2 * NT * SW_R;
     const int tpr = (int)((n_t + TILE - 1) / TILE);
@@ -875,16 +914,16 @@ static cudaError_t launch_sweep_nt(const float *x, int64_t n_dm, int64_t n_t, in
         const FusedSmem lay(nmax, NT);
         if ((e = persistent_grid(boxcar_search_fused<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
         boxcar_search_fused<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax,
-                                                                threshold, out, capacity, d_count);
+                                                                threshold, out, capacity, d_count, stats_stride);
     } else if (nmax <= SW_NARROW_NMAX) {
         const FusedSmem lay(nmax, NT);
         if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
         boxcar_snr_sweep_narrow<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width,
-                                                                    0, 1, row_stride);
+                                                                    0, 1, row_stride, stats_stride);
     } else {
         const SweepSmem lay(nmax, NT);
         if ((e = persistent_grid(boxcar_snr_sweep<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width);
+        boxcar_snr_sweep<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width, stats_stride);
     }
     return cudaGetLastError();
 }
@@ -893,14 +932,14 @@ static cudaError_t launch_sweep_nt(const float *x, int64_t n_dm, int64_t n_t, in
 cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
                          const float *d_table, int nmax, bool rc, float *snr, uint16_t *width,
                          bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
-                         unsigned long long *d_count, cudaStream_t s)
+                         unsigned long long *d_count, cudaStream_t s, int stats_stride)
 {
     if (nmax <= SW_SMALL_CTA_NMAX) {
-        if (rc) return launch_sweep_nt<64, true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
-        return launch_sweep_nt<64, false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
+        if (rc) return launch_sweep_nt<64, true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s, stats_stride);
+        return launch_sweep_nt<64, false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s, stats_stride);
     }
-    if (rc) return launch_sweep_nt<128, true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
-    return launch_sweep_nt<128, false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s);
+    if (rc) return launch_sweep_nt<128, true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s, stats_stride);
+    return launch_sweep_nt<128, false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s, stats_stride);
 }
 
 // one level of the decimated search: the narrow kernel on the decimated series x_l (w0 <= 32) with the level's statistics
@@ -917,10 +956,10 @@ cudaError_t launch_sweep_level(const float *xl, int64_t n_dm, int64_t n_l, int64
     cudaError_t e;
     if (rc) {
         if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, true>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep_narrow<NT, true><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride);
+        boxcar_snr_sweep_narrow<NT, true><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride, 0);
     } else {
         if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, false>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep_narrow<NT, false><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride);
+        boxcar_snr_sweep_narrow<NT, false><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride, 0);
     }
     return cudaGetLastError();
 }

@@ -83,3 +83,30 @@ def test_product_path_has_no_cpu_fallback():
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 assert "oracle" not in open(os.path.join(dirpath, f)).read(), f
+
+
+def test_round2_entry_points_validate_arguments(L):
+    """spd_stats_rows / spd_boxcar_snr_rows / spd_search_fused_rows / spd_boxcar_snr_decimated / spd_candidates_decimated."""
+    fake = C.c_void_p(4096)
+    INV, WS = 1, 3
+    L.spd_decimated_level_offset.restype = C.c_int64
+    L.spd_decimated_level_offset.argtypes = [C.c_int64, C.c_int]
+    L.spd_decimated_workspace_bytes.restype = C.c_size_t
+    assert [L.spd_decimated_level_offset(1003, l) for l in range(5)] == [0, 1008, 1512, 1768, 1896]     # rows of 1003, 501, 250, 125 padded to 8
+    assert L.spd_decimated_level_offset(0, 1) == -1
+    assert L.spd_decimated_workspace_bytes(C.c_int64(2), C.c_int64(4096), 16, 4) >= 2 * (2048 + 1024) * 4
+    assert L.spd_decimated_workspace_bytes(C.c_int64(2), C.c_int64(4096), 24, 4) == 0                      # w0 must be 16 or 32
+    assert L.spd_decimated_workspace_bytes(C.c_int64(2), C.c_int64(4096), 32, 9) == 0                      # 32 * 2^8 > 4096
+    a = [C.c_int64(2), C.c_int64(4096), C.c_int64(4096)]
+    assert L.spd_boxcar_snr_decimated(fake, *a, fake, 8, 2, 0, fake, fake, C.c_int64(8192), fake, C.c_size_t(1 << 30), None) == INV
+    assert L.spd_boxcar_snr_decimated(fake, *a, fake, 16, 2, 0, fake, fake, C.c_int64(100), fake, C.c_size_t(1 << 30), None) == INV   # plane_stride too short
+    assert L.spd_boxcar_snr_decimated(fake, *a, fake, 16, 2, 0, fake, fake, C.c_int64(8192), fake, C.c_size_t(64), None) == WS
+    assert L.spd_candidates_decimated(fake, fake, C.c_int64(2), C.c_int64(4096), C.c_int64(100), 2, C.c_float(5.0), fake, C.c_uint64(10), fake, None) == INV
+    L.spd_workspace_bytes_rows.restype = C.c_size_t
+    assert L.spd_workspace_bytes_rows(C.c_int64(100), C.c_int64(4096), 64) >= 100 * 80 * 4
+    assert L.spd_stats_rows(fake, C.c_int64(0), C.c_int64(10), C.c_int64(10), 0, fake, fake, C.c_size_t(1 << 20), None) == INV
+    assert L.spd_stats_rows(fake, C.c_int64(4), C.c_int64(10), C.c_int64(10), 0, fake, fake, C.c_size_t(16), None) == WS
+    assert L.spd_boxcar_snr_rows(fake, C.c_int64(4), C.c_int64(100), C.c_int64(100), fake, 101, 0, fake, fake, fake, C.c_size_t(1 << 20), None) == INV
+    assert L.spd_boxcar_snr_rows(fake, C.c_int64(4), C.c_int64(100), C.c_int64(100), fake, 40, 1, fake, fake, fake, C.c_size_t(64), None) == WS
+    assert L.spd_search_fused_rows(fake, C.c_int64(4), C.c_int64(100), C.c_int64(100), fake, 40, 0, C.c_float(float("nan")), fake, C.c_uint64(4), fake,
+                                   fake, C.c_size_t(1 << 20), None) == INV
