@@ -75,6 +75,21 @@ __device__ __forceinline__ void warp_merge_full(float &T, float &S)
     }
 }
 
+// eq. 2 for accumulator (+) one FULL 512-value warp chunk (T, S in fp32): the hot merge, once per warp
+// and tile.  Same quantity as tri_merge, (n T1 - m T2)^2 / (m n (m + n)), with the reciprocal of m n (m + n) taken in
+// fp32 instead of an fp64 division (a ~60-instruction subroutine): the term is the between-chunk correction, a small
+// fraction of S, so 1e-7 relative in it is orders of magnitude below the 1e-6 tolerance on sigma.
+__device__ __forceinline__ void tri_merge_chunk(Tri &a, float T, float S)
+{
+    const double n = 512.0;
+    if (a.m == 0.0) { a.m = n; a.T = (double)T; a.S = (double)S; return; }
+    const double d = n * a.T - a.m * (double)T;
+    const float rf = __frcp_rn((float)a.m * (float)(a.m + n));
+    a.S = a.S + (double)S + d * d * ((double)rf * (1.0 / 512.0));
+    a.T += (double)T;
+    a.m += n;
+}
+
 // runs of any length (ragged chunk): eq. 2 in fp64, the left operand always being the lower lanes
 __device__ __forceinline__ void warp_merge_ragged(Tri &t, int lane)
 {
@@ -172,7 +187,7 @@ stats_partial(const float *__restrict__ x, int64_t n_rows, int64_t n_t, int64_t 
             float T, S;
             chan_run16(v, T, S);
             warp_merge_full(T, S);
-            if (lane == 0) { Tri w = {512.0, (double)T, (double)S}; tri_merge(acc, w); }
+            if (lane == 0) tri_merge_chunk(acc, T, S);
         } else {
             // ragged / unaligned chunk: eq. 1 with a run-time j, eq. 2 merges in fp64
             int cnt = 0;
@@ -214,6 +229,114 @@ __device__ __forceinline__ void load16(const float *sm, int pos, float (&v)[ST_R
     }
 }
 
+// One tile of stats_partial_win.  FAST = interior tile of a 16-byte aligned row: all 4096 samples, the whole halo and all
+// 4096 windows exist, so every run is full and nothing needs masking (63 of 64 tiles of a 262144-sample row).
+template <bool FAST>
+__device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__restrict__ Ps, float (*wtot)[ST_THREADS / 32],
+                                         int64_t t0, int64_t n_t, int64_t nwin, int nmax, int span, int span4, int nparts, float K,
+                                         Tri &acc, Tri &accb)
+{
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int own = ST_RUN * tid;                              // first position of this thread inside the tile
+    float xo[ST_RUN];
+    load16(xs, own, xo);
+    int cnt = ST_RUN, wcnt = ST_RUN;
+    if (!FAST) {
+        const int64_t left = n_t - (t0 + own), wleft = nwin - (t0 + own);
+        cnt = left >= ST_RUN ? ST_RUN : (left > 0 ? (int)left : 0);      // valid samples from the thread's first position on
+        wcnt = wleft >= ST_RUN ? ST_RUN : (wleft > 0 ? (int)wleft : 0);  // full windows that start there
+    }
+
+    // ---- sample statistics (the tile's own 4096 positions) ----
+    float y[ST_RUN];
+#pragma unroll
+    for (int k = 0; k < ST_RUN; ++k) y[k] = xo[k] - K;
+    if (FAST || __all_sync(0xffffffffu, cnt == ST_RUN)) {
+        float T, S;
+        chan_run16(y, T, S);
+        warp_merge_full(T, S);
+        if (lane == 0) tri_merge_chunk(acc, T, S);
+    } else {
+        Tri t = chan_run_ragged(y, cnt);
+        warp_merge_ragged(t, lane);
+        if (lane == 0) tri_merge(acc, t);
+    }
+
+    // ---- exclusive prefix sums of x - K over tile + halo (positions past the row end hold x = 0 and are not used;
+    //      FAST: positions past the staged span hold stale finite-or-not values that only reach prefix entries nobody reads) ----
+    float carry = 0.f;
+    for (int part = 0; part < nparts; ++part) {
+        const int pos = part * ST_CHUNK + own;
+        const bool act = pos < span + ST_RUN;                  // this thread's 16 positions start inside the staged span (+1 group for P[span])
+        const bool wact = part == 0 || (pos - ST_RUN * lane) < span + ST_RUN;   // warp-uniform: any lane of this warp active
+        float v[ST_RUN];
+        float inc = 0.f;
+        if (wact) {
+            if (part == 0) {
+#pragma unroll
+                for (int k = 0; k < ST_RUN; ++k) v[k] = y[k];
+            } else if (act && pos < span4) {
+                load16(xs, pos, v);
+#pragma unroll
+                for (int k = 0; k < ST_RUN; ++k) v[k] = (FAST || pos + k < span) ? v[k] - K : 0.f;
+            } else {
+#pragma unroll
+                for (int k = 0; k < ST_RUN; ++k) v[k] = 0.f;
+            }
+#pragma unroll
+            for (int k = 1; k < ST_RUN; ++k) v[k] += v[k - 1];
+            inc = v[ST_RUN - 1];
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { const float o = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += o; }
+        } else {
+#pragma unroll
+            for (int k = 0; k < ST_RUN; ++k) v[k] = 0.f;
+        }
+        if (lane == 31) wtot[part & 1][wid] = inc;
+        __syncthreads();
+        float off = inc - v[ST_RUN - 1] + carry;
+        {
+            const float4 ta = *reinterpret_cast<const float4 *>(&wtot[part & 1][0]), tb = *reinterpret_cast<const float4 *>(&wtot[part & 1][4]);
+            const float t[8] = {ta.x, ta.y, ta.z, ta.w, tb.x, tb.y, tb.z, tb.w};
+#pragma unroll
+            for (int w = 0; w < ST_THREADS / 32; ++w) { if (w < wid) off += t[w]; carry += t[w]; }
+        }
+        if (act) {
+            float4 *dp = reinterpret_cast<float4 *>(Ps + st_pad(pos));      // E[pos + k] = off + v[k-1]
+            dp[0] = make_float4(off, off + v[0], off + v[1], off + v[2]);
+            dp[1] = make_float4(off + v[3], off + v[4], off + v[5], off + v[6]);
+            dp[2] = make_float4(off + v[7], off + v[8], off + v[9], off + v[10]);
+            dp[3] = make_float4(off + v[11], off + v[12], off + v[13], off + v[14]);
+        }
+    }
+    __syncthreads();
+
+    // ---- the 16 windows that start at the thread's positions ----
+    float b[ST_RUN];
+    if (FAST || wcnt > 0) {
+        b[0] = Ps[st_pad(own + nmax)] - Ps[st_pad(own)];
+        if ((nmax & 3) == 0) {                                 // the entering samples x[own + nmax + k] as four 16-byte loads
+            float e[ST_RUN];
+            load16(xs, own + nmax, e);
+#pragma unroll
+            for (int k = 1; k < ST_RUN; ++k) b[k] = b[k - 1] + (e[k - 1] - xo[k - 1]);
+        } else {
+#pragma unroll
+            for (int k = 1; k < ST_RUN; ++k) b[k] = b[k - 1] + (xs[st_pad(own + nmax + k - 1)] - xo[k - 1]);
+        }
+    }
+    if (FAST || __all_sync(0xffffffffu, wcnt == ST_RUN)) {
+        float T, S;
+        chan_run16(b, T, S);
+        warp_merge_full(T, S);
+        if (lane == 0) tri_merge_chunk(accb, T, S);
+    } else if (__any_sync(0xffffffffu, wcnt > 0)) {
+        Tri t = chan_run_ragged(b, wcnt);
+        warp_merge_ragged(t, lane);
+        if (lane == 0) tri_merge(accb, t);
+    }
+}
+
 __global__ void __launch_bounds__(ST_THREADS, 3)
 stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax,
                   Tri *__restrict__ part_x, Tri *__restrict__ part_b)
@@ -224,12 +347,13 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
     extern __shared__ __align__(16) unsigned char st_smem[];
     __shared__ Tri warp_acc[ST_THREADS / 32];
     __shared__ float red[2 * ST_THREADS / 32];
-    __shared__ float wtot[2][ST_THREADS / 32];
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    __shared__ __align__(16) float wtot[2][ST_THREADS / 32];
+    const int tid = threadIdx.x;
     const int span = ST_CHUNK + nmax - 1;                      // samples staged per tile
     const int span4 = (span + 3) & ~3;
-    float *xs = reinterpret_cast<float *>(st_smem);            // [st_pad(span4)] raw samples, 0 past the row end
-    float *Ps = xs + st_pad(span4 + ST_RUN);                   // [st_pad(span4 + 16)] exclusive prefix sums of x - K
+    const int xs_len = st_pad(span4 + ST_RUN);
+    float *xs0 = reinterpret_cast<float *>(st_smem);           // two landing buffers [st_pad(span4 + 16)]: raw samples, 0 past the row end
+    float *Ps = xs0 + 2 * xs_len;                              // [st_pad(span4 + 32)] exclusive prefix sums of x - K
     const int64_t nwin = n_t - nmax + 1;                       // full windows per row
     const int64_t tpr = (n_t + ST_CHUNK - 1) / ST_CHUNK;
     const int64_t total = n_dm * tpr;
@@ -238,120 +362,54 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
     float K = 0.f;
     bool have_K = false;
 
-    for (int64_t c = blockIdx.x; c < total; c += gridDim.x) {
+    auto interior = [&](int64_t c) {                           // whole tile + halo inside a 16-byte aligned row
+        const int64_t row = c / tpr, t0 = (c - row * tpr) * ST_CHUNK;
+        return ((reinterpret_cast<uintptr_t>(x + row * row_stride) & 15) == 0) && (t0 + span4 <= n_t);
+    };
+    // stage tile c into landing buffer `buf` (asynchronous 16-byte copies; scalar loads at the row end / for unaligned rows)
+    auto stage = [&](int64_t c, int buf) {
         const int64_t row = c / tpr, t0 = (c - row * tpr) * ST_CHUNK;
         const float *rp = x + row * row_stride;
-        const bool vec = ((reinterpret_cast<uintptr_t>(rp) & 15) == 0);
-        __syncthreads();                                       // everyone is done with the previous tile
-        for (int p = tid; p < span4 / 4; p += ST_THREADS) {
-            const int64_t pos = t0 + 4 * p;
-            float *dst = xs + st_pad(4 * p);
-            if (vec && pos + 3 < n_t) cp_async16_st(dst, rp + pos);
-            else {
+        float *xb = xs0 + buf * xs_len;
+        if (interior(c)) {
+            const float *src = rp + t0;
+            for (int p = tid; p < span4 / 4; p += ST_THREADS) cp_async16_st(xb + st_pad(4 * p), src + 4 * p);
+        } else {
+            const bool vec = ((reinterpret_cast<uintptr_t>(rp) & 15) == 0);
+            for (int p = tid; p < span4 / 4; p += ST_THREADS) {
+                const int64_t pos = t0 + 4 * p;
+                float *dst = xb + st_pad(4 * p);
+                if (vec && pos + 3 < n_t) cp_async16_st(dst, rp + pos);
+                else {
 #pragma unroll
-                for (int k = 0; k < 4; ++k) dst[k] = (pos + k < n_t) ? __ldg(rp + pos + k) : 0.0f;
+                    for (int k = 0; k < 4; ++k) dst[k] = (pos + k < n_t) ? __ldg(rp + pos + k) : 0.0f;
+                }
             }
         }
-        asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
-        __syncthreads();
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    int buf = 0;
+    if ((int64_t)blockIdx.x < total) stage(blockIdx.x, 0);
 
-        const int own = ST_RUN * tid;                          // first position of this thread inside the tile
-        float xo[ST_RUN];
-        load16(xs, own, xo);
-        int64_t left = n_t - (t0 + own);                       // valid samples from the thread's first position on
-        const int cnt = left >= ST_RUN ? ST_RUN : (left > 0 ? (int)left : 0);
+    for (int64_t c = blockIdx.x; c < total; c += gridDim.x, buf ^= 1) {
+        const int64_t row = c / tpr, t0 = (c - row * tpr) * ST_CHUNK;
+        const float *xs = xs0 + buf * xs_len;
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();                                       // this tile has landed; everyone is done with the previous tile (other buffer, Ps)
+        if (c + gridDim.x < total) stage(c + gridDim.x, buf ^ 1);   // the next tile streams in while this one is reduced
+
         if (!have_K) {                                         // shift of this CTA: the mean of its first tile
+            float xo[ST_RUN];
+            load16(xs, ST_RUN * tid, xo);
+            const int64_t left = n_t - (t0 + ST_RUN * tid);
+            const int cnt = left >= ST_RUN ? ST_RUN : (left > 0 ? (int)left : 0);
             float s = 0.f;
             for (int k = 0; k < ST_RUN; ++k) if (k < cnt) s += xo[k];
             K = cta_mean(s, (float)cnt, red);
             have_K = true;
         }
-
-        // ---- sample statistics (the tile's own 4096 positions) ----
-        float y[ST_RUN];
-#pragma unroll
-        for (int k = 0; k < ST_RUN; ++k) y[k] = xo[k] - K;
-        if (__all_sync(0xffffffffu, cnt == ST_RUN)) {
-            float T, S;
-            chan_run16(y, T, S);
-            warp_merge_full(T, S);
-            if (lane == 0) { Tri w = {512.0, (double)T, (double)S}; tri_merge(acc, w); }
-        } else {
-            Tri t = chan_run_ragged(y, cnt);
-            warp_merge_ragged(t, lane);
-            if (lane == 0) tri_merge(acc, t);
-        }
-
-        // ---- exclusive prefix sums of x - K over tile + halo (positions past the row end hold x = 0 and are not used) ----
-        float carry = 0.f;
-        for (int part = 0; part < nparts; ++part) {
-            const int pos = part * ST_CHUNK + own;
-            const bool act = pos < span4 + ST_RUN && pos < span + ST_RUN;        // this thread's 16 positions start inside the staged span (+1 group for P[span])
-            const bool wact = part == 0 || (pos - ST_RUN * lane) < span + ST_RUN;   // warp-uniform: any lane of this warp active
-            float v[ST_RUN];
-            float inc = 0.f;
-            if (wact) {
-                if (part == 0) {
-#pragma unroll
-                    for (int k = 0; k < ST_RUN; ++k) v[k] = y[k];
-                } else if (act && pos < span4) {
-                    load16(xs, pos, v);
-#pragma unroll
-                    for (int k = 0; k < ST_RUN; ++k) v[k] = (pos + k < span) ? v[k] - K : 0.f;
-                } else {
-#pragma unroll
-                    for (int k = 0; k < ST_RUN; ++k) v[k] = 0.f;
-                }
-#pragma unroll
-                for (int k = 1; k < ST_RUN; ++k) v[k] += v[k - 1];
-                inc = v[ST_RUN - 1];
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) { const float o = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += o; }
-            } else {
-#pragma unroll
-                for (int k = 0; k < ST_RUN; ++k) v[k] = 0.f;
-            }
-            if (lane == 31) wtot[part & 1][wid] = inc;
-            __syncthreads();
-            float off = inc - v[ST_RUN - 1] + carry;
-#pragma unroll
-            for (int w = 0; w < ST_THREADS / 32; ++w) { const float t = wtot[part & 1][w]; if (w < wid) off += t; carry += t; }
-            if (act) {
-                float4 *dp = reinterpret_cast<float4 *>(Ps + st_pad(pos));      // E[pos + k] = off + v[k-1]
-                dp[0] = make_float4(off, off + v[0], off + v[1], off + v[2]);
-                dp[1] = make_float4(off + v[3], off + v[4], off + v[5], off + v[6]);
-                dp[2] = make_float4(off + v[7], off + v[8], off + v[9], off + v[10]);
-                dp[3] = make_float4(off + v[11], off + v[12], off + v[13], off + v[14]);
-            }
-        }
-        __syncthreads();
-
-        // ---- the 16 windows that start at the thread's positions ----
-        int64_t wleft = nwin - (t0 + own);
-        const int wcnt = wleft >= ST_RUN ? ST_RUN : (wleft > 0 ? (int)wleft : 0);
-        float b[ST_RUN];
-        if (wcnt > 0) {
-            b[0] = Ps[st_pad(own + nmax)] - Ps[st_pad(own)];
-            if ((nmax & 3) == 0) {                             // the entering samples x[own + nmax + k] as four 16-byte loads
-                float e[ST_RUN];
-                load16(xs, own + nmax, e);
-#pragma unroll
-                for (int k = 1; k < ST_RUN; ++k) b[k] = b[k - 1] + (e[k - 1] - xo[k - 1]);
-            } else {
-#pragma unroll
-                for (int k = 1; k < ST_RUN; ++k) b[k] = b[k - 1] + (xs[st_pad(own + nmax + k - 1)] - xo[k - 1]);
-            }
-        }
-        if (__all_sync(0xffffffffu, wcnt == ST_RUN)) {
-            float T, S;
-            chan_run16(b, T, S);
-            warp_merge_full(T, S);
-            if (lane == 0) { Tri w = {512.0, (double)T, (double)S}; tri_merge(accb, w); }
-        } else if (__any_sync(0xffffffffu, wcnt > 0)) {
-            Tri t = chan_run_ragged(b, wcnt);
-            warp_merge_ragged(t, lane);
-            if (lane == 0) tri_merge(accb, t);
-        }
+        if (interior(c)) win_tile<true>(xs, Ps, wtot, t0, n_t, nwin, nmax, span, span4, nparts, K, acc, accb);
+        else win_tile<false>(xs, Ps, wtot, t0, n_t, nwin, nmax, span, span4, nparts, K, acc, accb);
     }
     write_partial(warp_acc, acc, (double)K, 1.0, part_x + blockIdx.x);
     write_partial(warp_acc, accb, (double)K, (double)nmax, part_b + blockIdx.x);
@@ -435,7 +493,7 @@ static cudaError_t stats_win_limit()
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64 || !limit_set[dev]) {
-        e = cudaFuncSetAttribute(stats_partial_win, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(2 * st_pad(ST_CHUNK + 4096 + 2 * ST_RUN) * sizeof(float)));
+        e = cudaFuncSetAttribute(stats_partial_win, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * st_pad(ST_CHUNK + 4096 + 2 * ST_RUN) * sizeof(float)));
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) limit_set[dev] = true;
     }
@@ -451,7 +509,7 @@ cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
         const int64_t tiles = n_dm * ((n_t + ST_CHUNK - 1) / ST_CHUNK);
         gx = gb = (int)(tiles < ST_GRID ? tiles : ST_GRID);
         const int span4 = (ST_CHUNK + nmax_for_sigma - 1 + 3) & ~3;
-        const size_t smem = (size_t)(st_pad(span4 + ST_RUN) + st_pad(span4 + 2 * ST_RUN)) * sizeof(float);
+        const size_t smem = (size_t)(2 * st_pad(span4 + ST_RUN) + st_pad(span4 + 2 * ST_RUN)) * sizeof(float);
         cudaError_t e = stats_win_limit();
         if (e != cudaSuccess) return e;
         stats_partial_win<<<gx, ST_THREADS, smem, s>>>(x, n_dm, n_t, row_stride, nmax_for_sigma, px, pb);
@@ -481,7 +539,7 @@ cudaError_t launch_stats_rows(const float *x, int64_t n_dm, int64_t n_t, int64_t
     if (nmax_for_sigma > 0) {
         if ((e = stats_win_limit()) != cudaSuccess) return e;
         const int span4 = (ST_CHUNK + nmax_for_sigma - 1 + 3) & ~3;
-        smem = (size_t)(st_pad(span4 + ST_RUN) + st_pad(span4 + 2 * ST_RUN)) * sizeof(float);
+        smem = (size_t)(2 * st_pad(span4 + ST_RUN) + st_pad(span4 + 2 * ST_RUN)) * sizeof(float);
     }
     for (int64_t r0 = 0; r0 < n_dm; r0 += 65535) {               // grid.y limit
         const unsigned ny = (unsigned)(n_dm - r0 < 65535 ? n_dm - r0 : 65535);

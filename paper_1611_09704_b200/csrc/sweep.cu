@@ -57,7 +57,7 @@ constexpr int SW_SMALL_CTA_NMAX = 256;
 constexpr int SW_NARROW_NMAX = 32;                   // nmax up to here takes the tagged-maximum kernel (5 tag bits)
 constexpr int SW_NMAX_TAB = 4096 + 16;               // entries of the constant 1/sqrt(w) table (API limit of nmax + padding)
 
-__host__ __device__ inline int zpad(int i) { return i + (i >> 3); }          // one pad float2 per 8: lane stride 72 B
+__host__ __device__ inline int zpad(int i) { return i + ((i >> 3) << 1); }   // two pad float2 per 8: lane stride 80 B, conflict-free 16-byte accesses
 __host__ __device__ inline int sw_nblk(int nmax) { return (nmax + 7) >> 3; }  // blocks of 8 widths
 __host__ __device__ inline int sw_halo(int nmax) { return 8 * sw_nblk(nmax) + 8; }   // positions staged past a sub-tile
 __host__ __device__ inline int sw_rt_len(int nmax) { return 8 * sw_nblk(nmax) + 8; } // reciprocal-table entries
@@ -305,6 +305,14 @@ __device__ __forceinline__ void load_group(const float *raw, int g, float2 (&v)[
     v[4] = make_float2(a1.x, b1.x); v[5] = make_float2(a1.y, b1.y); v[6] = make_float2(a1.z, b1.z); v[7] = make_float2(a1.w, b1.w);
 }
 
+// group g of the working layout: Z[zpad(8 g + j)] = v[j], four 16-byte stores (zpad(8 g) = 10 g)
+__device__ __forceinline__ void store_group(float2 *Z, int g, const float2 (&v)[SW_R])
+{
+    float4 *d = reinterpret_cast<float4 *>(Z + 10 * g);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) d[k] = make_float4(v[2 * k].x, v[2 * k].y, v[2 * k + 1].x, v[2 * k + 1].y);
+}
+
 // One block of 8 width steps: advance the 8 packed running sums, scale, fold into the running maxima.
 // out[j] = max(in[j], the 8 SNRs of this block); `in` stays intact so that the caller can tell whether the block
 // raised the maximum.  On entry W[v] = Z[8 tid + a0 + v] (a0 = width offset of the first step); on exit the window
@@ -321,7 +329,8 @@ __device__ __forceinline__ void sweep8(float2 (&B)[SW_R], float2 (&W)[SW_R], con
         if (RC) rr = make_float2(c_isqrt.v[w0 + u], c_isqrt.v[w0 + u + 1]);
         else rr = *reinterpret_cast<const float2 *>(rp + u);
         const float2 r0 = make_float2(rr.x, rr.x), r1 = make_float2(rr.y, rr.y);
-        const float2 n0 = zp[u], n1 = zp[u + 1];
+        const float4 nq = *reinterpret_cast<const float4 *>(zp + u);     // two window elements per 16-byte load
+        const float2 n0 = make_float2(nq.x, nq.y), n1 = make_float2(nq.z, nq.w);
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) {
             B[j] = __fadd2_rn(B[j], W[(j + u) & 7]);
@@ -491,10 +500,8 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
                     if (act) {
                         load_group<SW_SUB>(raw, g, v);
 #pragma unroll
-                        for (int j = 0; j < SW_R; ++j) {
-                            v[j] = norm.apply<RC>(v[j]);
-                            Z[9 * g + j] = v[j];                 // zpad(8 g + j) = 9 g + j
-                        }
+                        for (int j = 0; j < SW_R; ++j) v[j] = norm.apply<RC>(v[j]);
+                        store_group(Z, g, v);
                     } else {
 #pragma unroll
                         for (int j = 0; j < SW_R; ++j) v[j] = make_float2(0.f, 0.f);
@@ -539,7 +546,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
 
         // ---- main loop: blocks of 8 widths, the running maximum ping-pongs between bestA and bestB ---------------------
         {
-            const float2 *zp = Z + 9 * (tid + 1);                // zpad(8 tid + 8 kb + 8 + u) = 9 (tid + kb + 1) + u
+            const float2 *zp = Z + 10 * (tid + 1);               // zpad(8 tid + 8 kb + 8 + u) = 10 (tid + kb + 1) + u
             const float *rp = rtf;
             int kb = 0;
             int kbv = opaque_reg(0);      // the block index as a per-thread value for note_block: the loop counter itself stays
@@ -547,9 +554,9 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
             for (; kb + 2 <= nblk; kb += 2, kbv += 2) {
                 sweep8<RC>(B, W, bestA, bestB, zp, rp, 8 * kb);
                 note_block(bestB, bestA, kbv, kx, ky);
-                sweep8<RC>(B, W, bestB, bestA, zp + 9, rp + 8, 8 * kb + 8);
+                sweep8<RC>(B, W, bestB, bestA, zp + 10, rp + 8, 8 * kb + 8);
                 note_block(bestA, bestB, kbv + 1, kx, ky);
-                zp += 18; rp += 16;
+                zp += 20; rp += 16;
             }
             if (kb < nblk) {
                 sweep8<RC>(B, W, bestA, bestB, zp, rp, 8 * kb);
@@ -674,9 +681,9 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
 #pragma unroll
                 for (int j = 0; j < SW_R; ++j) {
                     v[j] = norm.apply<RC>(v[j]);
-                    Z[9 * g + j] = v[j];
                     if (part == 0) W[j] = v[j];
                 }
+                store_group(Z, g, v);
             }
         }
         __syncthreads();                           // Z complete; raw is free again
@@ -685,12 +692,12 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); }
         {
-            const float2 *zp = Z + 9 * (tid + 1);
+            const float2 *zp = Z + 10 * (tid + 1);
             const float *rp = rtf;
             int kb = 0;
-            for (; kb + 2 <= nblk; kb += 2, zp += 18, rp += 16) {
+            for (; kb + 2 <= nblk; kb += 2, zp += 20, rp += 16) {
                 sweep8<RC>(B, W, best, best, zp, rp, 8 * kb);
-                sweep8<RC>(B, W, best, best, zp + 9, rp + 8, 8 * kb + 8);
+                sweep8<RC>(B, W, best, best, zp + 10, rp + 8, 8 * kb + 8);
             }
             if (kb < nblk) sweep8<RC>(B, W, best, best, zp, rp, 8 * kb);
         }
@@ -736,7 +743,8 @@ __device__ __forceinline__ void sweep8_tagged(float2 (&B)[SW_R], float2 (&W)[SW_
         if (RC) rr = make_float2(c_isqrt.v[8 * KB + u], c_isqrt.v[8 * KB + u + 1]);
         else rr = *reinterpret_cast<const float2 *>(rp + u);
         const float2 r0 = make_float2(rr.x, rr.x), r1 = make_float2(rr.y, rr.y);
-        const float2 n0 = zp[u], n1 = zp[u + 1];
+        const float4 nq = *reinterpret_cast<const float4 *>(zp + u);     // two window elements per 16-byte load
+        const float2 n0 = make_float2(nq.x, nq.y), n1 = make_float2(nq.z, nq.w);
         const int c0 = 32 - (8 * KB + u + 1), c1 = c0 - 1;              // 32 - w for the two widths of this step
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) {
@@ -813,9 +821,9 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
 #pragma unroll
                 for (int j = 0; j < SW_R; ++j) {
                     v[j] = norm.apply<RC>(v[j]);
-                    Z[9 * g + j] = v[j];
                     if (part == 0) W[j] = v[j];
                 }
+                store_group(Z, g, v);
             }
         }
         __syncthreads();                           // Z complete; raw is free again
@@ -823,15 +831,15 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
 
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); tbest[j] = make_float2(NINF, NINF); }
-        const float2 *zp = Z + 9 * (tid + 1);
+        const float2 *zp = Z + 10 * (tid + 1);
         if (wmin >= 8) sweep8_tagged<0, RC, false>(B, W, best, tbest, zp, rtf, mask31);
         else sweep8_tagged<0, RC, true>(B, W, best, tbest, zp, rtf, mask31);
         if (nblk > 1) {
-            if (wmin >= 16) sweep8_tagged<1, RC, false>(B, W, best, tbest, zp + 9, rtf + 8, mask31);
-            else sweep8_tagged<1, RC, true>(B, W, best, tbest, zp + 9, rtf + 8, mask31);
+            if (wmin >= 16) sweep8_tagged<1, RC, false>(B, W, best, tbest, zp + 10, rtf + 8, mask31);
+            else sweep8_tagged<1, RC, true>(B, W, best, tbest, zp + 10, rtf + 8, mask31);
         }
-        if (nblk > 2) sweep8_tagged<2, RC, true>(B, W, best, tbest, zp + 18, rtf + 16, mask31);
-        if (nblk > 3) sweep8_tagged<3, RC, true>(B, W, best, tbest, zp + 27, rtf + 24, mask31);
+        if (nblk > 2) sweep8_tagged<2, RC, true>(B, W, best, tbest, zp + 20, rtf + 16, mask31);
+        if (nblk > 3) sweep8_tagged<3, RC, true>(B, W, best, tbest, zp + 30, rtf + 24, mask31);
 
         int wx[SW_R], wy[SW_R];
 #pragma unroll
