@@ -173,9 +173,19 @@ stats_partial(const float *__restrict__ x, int64_t n_rows, int64_t n_t, int64_t 
         K = cta_mean(s, cn, red);
     }
 
+    // (row, chunk-in-row) advanced with 32-bit arithmetic where the chunk count allows it
+    const bool small = cpr < 0x7fffffffLL;
+    int64_t row = (int64_t)blockIdx.x / cpr;
+    int64_t cir = (int64_t)blockIdx.x - row * cpr;
     for (int64_t c = blockIdx.x; c < total; c += gridDim.x) {
-        const int64_t row = c / cpr, off = (c - row * cpr) * ST_CHUNK;
-        const float *base = x + row * row_stride + off;
+        const int64_t off = cir * ST_CHUNK;
+        const int64_t row_now = row;
+        if (small) {
+            unsigned t = (unsigned)cir + gridDim.x;
+            if (t >= (unsigned)cpr) { const unsigned q = t / (unsigned)cpr; row += q; t -= q * (unsigned)cpr; }
+            cir = t;
+        } else { const int64_t cn = c + gridDim.x; row = cn / cpr; cir = cn - row * cpr; }
+        const float *base = x + row_now * row_stride + off;
         const bool full = (off + ST_CHUNK <= n_t) && ((reinterpret_cast<uintptr_t>(base) & 15) == 0);
         float v[ST_RUN];
         if (full) {
@@ -195,7 +205,7 @@ stats_partial(const float *__restrict__ x, int64_t n_rows, int64_t n_t, int64_t 
             for (int k = 0; k < ST_RUN; ++k) {                 // positions ascend with k, so the valid samples are a prefix of the run
                 const int64_t p = off + (int64_t)((k >> 2) * ST_THREADS + tid) * 4 + (k & 3);
                 const bool ok = p < n_t;
-                v[k] = ok ? __ldg(x + row * row_stride + p) - K : 0.0f;
+                v[k] = ok ? __ldg(x + row_now * row_stride + p) - K : 0.0f;
                 cnt += ok ? 1 : 0;
             }
             Tri t = chan_run_ragged(v, cnt);
@@ -295,11 +305,13 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
         if (lane == 31) wtot[part & 1][wid] = inc;
         __syncthreads();
         float off = inc - v[ST_RUN - 1] + carry;
-        {
-            const float4 ta = *reinterpret_cast<const float4 *>(&wtot[part & 1][0]), tb = *reinterpret_cast<const float4 *>(&wtot[part & 1][4]);
-            const float t[8] = {ta.x, ta.y, ta.z, ta.w, tb.x, tb.y, tb.z, tb.w};
+        {   // exclusive scan of the 8 warp totals by the first 8 lanes of every warp (3 shuffle steps), then two broadcasts
+            float t = wtot[part & 1][lane & 7];
 #pragma unroll
-            for (int w = 0; w < ST_THREADS / 32; ++w) { if (w < wid) off += t[w]; carry += t[w]; }
+            for (int d = 1; d < 8; d <<= 1) { const float o = __shfl_up_sync(0xffffffffu, t, d); if ((lane & 7) >= d) t += o; }
+            const float below = __shfl_sync(0xffffffffu, t, (wid + 7) & 7);      // inclusive total of warps 0..wid-1 (lane wid-1)
+            if (wid > 0) off += below;
+            carry += __shfl_sync(0xffffffffu, t, 7);
         }
         if (act) {
             float4 *dp = reinterpret_cast<float4 *>(Ps + st_pad(pos));      // E[pos + k] = off + v[k-1]
@@ -362,16 +374,25 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
     float K = 0.f;
     bool have_K = false;
 
-    auto interior = [&](int64_t c) {                           // whole tile + halo inside a 16-byte aligned row
-        const int64_t row = c / tpr, t0 = (c - row * tpr) * ST_CHUNK;
-        return ((reinterpret_cast<uintptr_t>(x + row * row_stride) & 15) == 0) && (t0 + span4 <= n_t);
+    // (row, tile-in-row) of the persistent walk, advanced by the grid size with 32-bit arithmetic (a 64-bit division per
+    // tile costs more instructions than the tile's arithmetic)
+    struct Pos { int64_t row; unsigned tr; };
+    const unsigned utpr = (unsigned)tpr;
+    auto advance = [&](Pos p) {
+        unsigned t = p.tr + gridDim.x;
+        if (t >= utpr) { const unsigned q = t / utpr; p.row += q; t -= q * utpr; }
+        p.tr = t;
+        return p;
     };
-    // stage tile c into landing buffer `buf` (asynchronous 16-byte copies; scalar loads at the row end / for unaligned rows)
-    auto stage = [&](int64_t c, int buf) {
-        const int64_t row = c / tpr, t0 = (c - row * tpr) * ST_CHUNK;
+    auto interior = [&](const Pos &p) {                        // whole tile + halo inside a 16-byte aligned row
+        return ((reinterpret_cast<uintptr_t>(x + p.row * row_stride) & 15) == 0) && ((int64_t)p.tr * ST_CHUNK + span4 <= n_t);
+    };
+    // stage a tile into landing buffer `buf` (asynchronous 16-byte copies; scalar loads at the row end / for unaligned rows)
+    auto stage = [&](const Pos &p, int buf) {
+        const int64_t row = p.row, t0 = (int64_t)p.tr * ST_CHUNK;
         const float *rp = x + row * row_stride;
         float *xb = xs0 + buf * xs_len;
-        if (interior(c)) {
+        if (interior(p)) {
             const float *src = rp + t0;
             for (int p = tid; p < span4 / 4; p += ST_THREADS) cp_async16_st(xb + st_pad(4 * p), src + 4 * p);
         } else {
@@ -389,14 +410,17 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     int buf = 0;
-    if ((int64_t)blockIdx.x < total) stage(blockIdx.x, 0);
+    Pos pos = {(int64_t)(blockIdx.x / utpr), blockIdx.x % utpr};
+    if ((int64_t)blockIdx.x < total) stage(pos, 0);
 
     for (int64_t c = blockIdx.x; c < total; c += gridDim.x, buf ^= 1) {
-        const int64_t row = c / tpr, t0 = (c - row * tpr) * ST_CHUNK;
+        const Pos cur = pos;
+        const int64_t t0 = (int64_t)cur.tr * ST_CHUNK;
+        pos = advance(pos);
         const float *xs = xs0 + buf * xs_len;
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();                                       // this tile has landed; everyone is done with the previous tile (other buffer, Ps)
-        if (c + gridDim.x < total) stage(c + gridDim.x, buf ^ 1);   // the next tile streams in while this one is reduced
+        if (c + gridDim.x < total) stage(pos, buf ^ 1);        // the next tile streams in while this one is reduced
 
         if (!have_K) {                                         // shift of this CTA: the mean of its first tile
             float xo[ST_RUN];
@@ -408,7 +432,7 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
             K = cta_mean(s, (float)cnt, red);
             have_K = true;
         }
-        if (interior(c)) win_tile<true>(xs, Ps, wtot, t0, n_t, nwin, nmax, span, span4, nparts, K, acc, accb);
+        if (interior(cur)) win_tile<true>(xs, Ps, wtot, t0, n_t, nwin, nmax, span, span4, nparts, K, acc, accb);
         else win_tile<false>(xs, Ps, wtot, t0, n_t, nwin, nmax, span, span4, nparts, K, acc, accb);
     }
     write_partial(warp_acc, acc, (double)K, 1.0, part_x + blockIdx.x);
