@@ -346,7 +346,9 @@ def run_ours(args):
     ws = P.new_workspace(n_dm, n_t, nmax, dev)
     out, cnt = P.new_candidates(cap, dev)
     nmax_sigma = nmax if mode != "sqrt" else 0
-    launches_per_step = 2 + (1 if nmax_sigma else 0) + 2 + 2     # stats(+sigma_nmax), table+sweep, zero+compact
+    # our kernels per step: stats_partial[_win] + stats_finalize, [sigma_table_kernel unless eq. 4 with nmax % 8 == 0], sweep,
+    # zero_count + candidates_compact (shard mode adds stats_merge_kernel)
+    launches_per_step = 2 + (0 if (mode == "sqrt" and nmax % 8 == 0) else 1) + 1 + 2 + (1 if shard_rows else 0)
 
     def step(ev=None):
         if shard_rows:     # local Chan triples, all-gather of the 80-byte structs (NCCL), eq. 2 fold in rank order: whole-chunk mu, sigma
