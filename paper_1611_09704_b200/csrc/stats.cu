@@ -279,6 +279,7 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
         const int pos = part * ST_CHUNK + own;
         const bool act = pos < span + ST_RUN;                  // this thread's 16 positions start inside the staged span (+1 group for P[span])
         const bool wact = part == 0 || (pos - ST_RUN * lane) < span + ST_RUN;   // warp-uniform: any lane of this warp active
+        if (!wact) { __syncthreads(); continue; }              // a warp past the staged span has nothing to add (nor in any later part)
         float v[ST_RUN];
         float inc = 0.f;
         if (wact) {
