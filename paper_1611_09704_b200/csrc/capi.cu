@@ -212,18 +212,17 @@ spd_status spd_boxcar_snr_decimated(const float *d_x, int64_t n_dm, int64_t n_t,
     for (int l = 0; l < levels; ++l) {
         const int D = 1 << l;
         const int64_t n_l = dec_n(n_t, l);
-        if (l > 0) {                                              // x_l = pairwise sums of x_{l-1}; the two buffers alternate
-            float *dst = buf[(l - 1) & 1];
-            const int64_t dst_stride = dec_stride(n_l);
-            if (launch_decimate2(src, n_dm, n_l, src_stride, dst, dst_stride, s) != cudaSuccess) return SPD_ERR_CUDA;
-            src = dst; src_stride = dst_stride;
-        }
         if (n_l < 1) break;
+        // the sweep of level l also writes x_{l+1} (pairwise sums of the tile it has staged anyway); the two buffers alternate
+        float *nxt = nullptr;
+        int64_t nxt_stride = 0;
+        if (l + 1 < levels && dec_n(n_t, l + 1) >= 1) { nxt = buf[l & 1]; nxt_stride = dec_stride(dec_n(n_t, l + 1)); }
         if (launch_level_stats(d_stats, D, lst, s) != cudaSuccess) return SPD_ERR_CUDA;
         if (!rc && launch_sigma_table(d_stats, w0, (int)mode, table, s, D, nmax_total) != cudaSuccess) return SPD_ERR_CUDA;
         const int64_t off = dec_off(n_t, l);
         if (launch_sweep_level(src, n_dm, n_l, src_stride, lst, table, w0, l == 0 ? 0 : w0 / 2, D, rc, d_snr + off, d_width + off,
-                               plane_stride, s) != cudaSuccess) return SPD_ERR_CUDA;
+                               plane_stride, nxt, nxt_stride, s) != cudaSuccess) return SPD_ERR_CUDA;
+        src = nxt; src_stride = nxt_stride;
     }
     return SPD_OK;
 }

@@ -47,11 +47,10 @@ size_t stats_rows_ws_bytes(int64_t n_dm);
 cudaError_t launch_stats_merge(const spd_stats_t *parts, int count, spd_stats_t *out, cudaStream_t s);
 cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, float *d_table, cudaStream_t s,
                                int wscale = 1, int nmax_total = 0, int64_t rows = 1);
-cudaError_t launch_decimate2(const float *src, int64_t n_dm, int64_t n_l, int64_t src_stride, float *dst, int64_t dst_stride, cudaStream_t s);
 cudaError_t launch_level_stats(const spd_stats_t *st, int D, spd_stats_t *out, cudaStream_t s);
 cudaError_t launch_sweep_level(const float *xl, int64_t n_dm, int64_t n_l, int64_t xl_stride, const spd_stats_t *d_stats_level,
                                const float *d_table, int w0, int wmin, int wscale, bool rc, float *snr, uint16_t *width,
-                               int64_t out_stride, cudaStream_t s);
+                               int64_t out_stride, float *dec_out, int64_t dec_stride, cudaStream_t s);
 bool sweep_uses_constant_table(int nmax, int mode);      // eq. 4 with nmax a multiple of 8: r_w = 1/sqrt(w) from the constant bank, no table launch
 cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
                          const float *d_table, int nmax, bool rc, float *snr, uint16_t *width,

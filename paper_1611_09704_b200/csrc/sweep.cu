@@ -147,41 +147,12 @@ cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, f
 // ---- decimation in time (reading A20): x_l[i] = x_{l-1}[2i] + x_{l-1}[2i+1]; the statistics of a level are those
 // of x scaled to sums of D = 2^l samples: mean_l = D mu, sigma_l = sqrt(D) sigma (eq. 3), so that eq. 4 of the decimated
 // series at width w' IS eq. 4 of x at the effective width w' D.  Nothing is re-measured.
-__global__ void decimate2_kernel(const float *__restrict__ src, int64_t n_dm, int64_t n_l, int64_t src_stride,
-                                 float *__restrict__ dst, int64_t dst_stride)
-{
-    const int64_t q4 = (n_l + 3) / 4;                           // groups of 4 outputs per row
-    const int64_t total = n_dm * q4;
-    for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t row = g / q4, i = (g - row * q4) * 4;
-        const float *sp = src + row * src_stride + 2 * i;
-        float *dp = dst + row * dst_stride + i;
-        if (i + 3 < n_l && ((reinterpret_cast<uintptr_t>(sp) & 15) == 0) && ((reinterpret_cast<uintptr_t>(dp) & 15) == 0)) {
-            float4 a, b;
-            asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w) : "l"(sp));
-            asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w) : "l"(sp + 4));
-            *reinterpret_cast<float4 *>(dp) = make_float4(__fadd_rn(a.x, a.y), __fadd_rn(a.z, a.w), __fadd_rn(b.x, b.y), __fadd_rn(b.z, b.w));
-        } else {
-            for (int k = 0; k < 4 && i + k < n_l; ++k) dp[k] = __fadd_rn(__ldg(sp + 2 * k), __ldg(sp + 2 * k + 1));
-        }
-    }
-}
-
 __global__ void level_stats_kernel(const spd_stats_t *__restrict__ st, int D, spd_stats_t *__restrict__ out)
 {
     spd_stats_t s = *st;
     s.mean = st->mean * (double)D;
     s.sigma = st->sigma * sqrt((double)D);
     *out = s;
-}
-
-cudaError_t launch_decimate2(const float *src, int64_t n_dm, int64_t n_l, int64_t src_stride, float *dst, int64_t dst_stride, cudaStream_t s)
-{
-    const int64_t groups = n_dm * ((n_l + 3) / 4);
-    if (groups <= 0) return cudaSuccess;
-    const int64_t blocks = (groups + 255) / 256;
-    decimate2_kernel<<<(unsigned)(blocks < 148 * 16 ? blocks : 148 * 16), 256, 0, s>>>(src, n_dm, n_l, src_stride, dst, dst_stride);
-    return cudaGetLastError();
 }
 
 cudaError_t launch_level_stats(const spd_stats_t *st, int D, spd_stats_t *out, cudaStream_t s)
@@ -763,14 +734,16 @@ __device__ __forceinline__ void sweep8_tagged(float2 (&B)[SW_R], float2 (&W)[SW_
     }
 }
 
-template <int SW_THREADS, bool RC>
+template <int SW_THREADS, bool RC, bool DEC>
 __global__ void __launch_bounds__(SW_THREADS, 640 / SW_THREADS)
 boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                         const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax,
                         float *__restrict__ snr, uint16_t *__restrict__ width,
                         int wmin /* widths <= wmin are summed but not evaluated (0 or a multiple of 8) */,
                         int wscale /* reported width = w * wscale */, int64_t out_stride /* row stride of the planes */,
-                        int stats_stride)
+                        int stats_stride,
+                        float *__restrict__ dec_out /* may be NULL: the next decimated level, x'[i] = x[2i] + x[2i+1] */,
+                        int64_t dec_stride)
 {
     constexpr int SW_SUB = SW_THREADS * SW_R, SW_TILE = 2 * SW_SUB;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -818,6 +791,18 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
             if (8 * g < LZ) {
                 float2 v[SW_R];
                 load_group<SW_SUB>(raw, g, v);
+                if (DEC && dec_out != nullptr && part == 0) {         // the tile's own samples, summed in pairs: the next level's series
+                    const int64_t n_next = n_t >> 1;
+                    const int64_t ia = (T0 + SW_R * tid) >> 1, ib = ia + SW_SUB / 2;
+                    float *da = dec_out + row * dec_stride + ia, *db = dec_out + row * dec_stride + ib;
+                    const float4 sa = make_float4(__fadd_rn(v[0].x, v[1].x), __fadd_rn(v[2].x, v[3].x), __fadd_rn(v[4].x, v[5].x), __fadd_rn(v[6].x, v[7].x));
+                    const float4 sb = make_float4(__fadd_rn(v[0].y, v[1].y), __fadd_rn(v[2].y, v[3].y), __fadd_rn(v[4].y, v[5].y), __fadd_rn(v[6].y, v[7].y));
+                    const bool al = ((reinterpret_cast<uintptr_t>(dec_out + row * dec_stride) & 15) == 0);
+                    if (al && ia + 3 < n_next) *reinterpret_cast<float4 *>(da) = sa;
+                    else { const float t[4] = {sa.x, sa.y, sa.z, sa.w}; for (int k = 0; k < 4; ++k) if (ia + k < n_next) da[k] = t[k]; }
+                    if (al && ib + 3 < n_next) *reinterpret_cast<float4 *>(db) = sb;
+                    else { const float t[4] = {sb.x, sb.y, sb.z, sb.w}; for (int k = 0; k < 4; ++k) if (ib + k < n_next) db[k] = t[k]; }
+                }
 #pragma unroll
                 for (int j = 0; j < SW_R; ++j) {
                     v[j] = norm.apply<RC>(v[j]);
@@ -925,9 +910,9 @@ static cudaError_t launch_sweep_nt(const float *x, int64_t n_dm, int64_t n_t, in
                                                                 threshold, out, capacity, d_count, stats_stride);
     } else if (nmax <= SW_NARROW_NMAX) {
         const FusedSmem lay(nmax, NT);
-        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep_narrow<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width,
-                                                                    0, 1, row_stride, stats_stride);
+        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, RC, false>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep_narrow<NT, RC, false><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width,
+                                                                    0, 1, row_stride, stats_stride, nullptr, 0);
     } else {
         const SweepSmem lay(nmax, NT);
         if ((e = persistent_grid(boxcar_snr_sweep<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
@@ -953,7 +938,7 @@ cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
 // one level of the decimated search: the narrow kernel on the decimated series x_l (w0 <= 32) with the level's statistics
 cudaError_t launch_sweep_level(const float *xl, int64_t n_dm, int64_t n_l, int64_t xl_stride, const spd_stats_t *d_stats_level,
                                const float *d_table, int w0, int wmin, int wscale, bool rc, float *snr, uint16_t *width,
-                               int64_t out_stride, cudaStream_t s)
+                               int64_t out_stride, float *dec_out, int64_t dec_stride, cudaStream_t s)
 {
     constexpr int NT = 64, TILE = 2 * NT * SW_R;
     if (n_l <= 0) return cudaSuccess;
@@ -963,11 +948,11 @@ cudaError_t launch_sweep_level(const float *xl, int64_t n_dm, int64_t n_l, int64
     unsigned grid = 0;
     cudaError_t e;
     if (rc) {
-        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, true>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep_narrow<NT, true><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride, 0);
+        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, true, true>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep_narrow<NT, true, true><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride, 0, dec_out, dec_stride);
     } else {
-        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, false>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_snr_sweep_narrow<NT, false><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride, 0);
+        if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, false, true>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep_narrow<NT, false, true><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride, 0, dec_out, dec_stride);
     }
     return cudaGetLastError();
 }
