@@ -53,7 +53,11 @@ constexpr int SW_R       = 8;                        // samples per thread per s
 // CTA width NT (a template parameter of the kernels): sub-tile = 8 NT samples, tile = 16 NT samples of one row.
 // 64 threads (tile 1024) for nmax <= SW_SMALL_CTA_NMAX: fewer warps wait on each block barrier; 128 threads (tile 2048)
 // above, where the halo (nmax + 8 positions staged and scanned per tile) would weigh too much on a small tile.
+// The general plane kernel runs ONE-warp CTAs (tile 512) up to SW_WARP_CTA_NMAX: its three block barriers per tile then
+// cost nothing (measured on the config-3 shape: Nmax 64 12.87 -> 12.54 ms, Nmax 128 20.39 -> 20.09 ms; Nmax 256 is slower,
+// and the fused and narrow kernels, which have a single barrier per tile, do not move).
 constexpr int SW_SMALL_CTA_NMAX = 256;
+constexpr int SW_WARP_CTA_NMAX = 128;
 constexpr int SW_NARROW_NMAX = 32;                   // nmax up to here takes the tagged-maximum kernel (5 tag bits)
 constexpr int SW_NMAX_TAB = 4096 + 16;               // entries of the constant 1/sqrt(w) table (API limit of nmax + padding)
 
@@ -903,7 +907,11 @@ static cudaError_t launch_sweep_nt(const float *x, int64_t n_dm, int64_t n_t, in
     const int64_t tiles = n_dm * (int64_t)tpr;
     unsigned grid = 0;
     cudaError_t e;
-    if (fused) {
+    if constexpr (NT == 32) {                      // one-warp CTAs: the general plane kernel only
+        const SweepSmem lay(nmax, NT);
+        if ((e = persistent_grid(boxcar_snr_sweep<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_snr_sweep<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax, snr, width, stats_stride);
+    } else if (fused) {
         const FusedSmem lay(nmax, NT);
         if ((e = persistent_grid(boxcar_search_fused<NT, RC>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
         boxcar_search_fused<NT, RC><<<grid, NT, lay.total, s>>>(x, n_t, row_stride, tpr, tiles, d_stats, d_table, nmax,
@@ -927,6 +935,10 @@ cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
                          bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
                          unsigned long long *d_count, cudaStream_t s, int stats_stride)
 {
+    if (!fused && nmax > SW_NARROW_NMAX && nmax <= SW_WARP_CTA_NMAX) {       // general plane kernel, one-warp CTAs
+        if (rc) return launch_sweep_nt<32, true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s, stats_stride);
+        return launch_sweep_nt<32, false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s, stats_stride);
+    }
     if (nmax <= SW_SMALL_CTA_NMAX) {
         if (rc) return launch_sweep_nt<64, true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s, stats_stride);
         return launch_sweep_nt<64, false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s, stats_stride);
