@@ -90,6 +90,19 @@ __device__ __forceinline__ void tri_merge_chunk(Tri &a, float T, float S)
     a.m += n;
 }
 
+// eq. 2 for a lane's own accumulator (+) one FULL 16-value run of the same lane (stats_partial_win: every lane keeps its
+// accumulator in fp64 across tiles, so a tile needs no shuffles; the lanes are merged once, when the CTA writes its partial)
+__device__ __forceinline__ void tri_merge_run(Tri &a, float T, float S)
+{
+    const double n = (double)ST_RUN;
+    if (a.m == 0.0) { a.m = n; a.T = (double)T; a.S = (double)S; return; }
+    const double d = n * a.T - a.m * (double)T;
+    const float rf = __frcp_rn((float)a.m * (float)(a.m + n));          // m (m + n) <= 2^24 * 16 stays well inside fp32's range
+    a.S = a.S + (double)S + d * d * ((double)rf * (1.0 / (double)ST_RUN));
+    a.T += (double)T;
+    a.m += n;
+}
+
 // runs of any length (ragged chunk): eq. 2 in fp64, the left operand always being the lower lanes
 __device__ __forceinline__ void warp_merge_ragged(Tri &t, int lane)
 {
@@ -133,10 +146,12 @@ __device__ __forceinline__ float cta_mean(float s, float c, float *sh)
     return Cn > 0.f ? S / Cn : 0.f;
 }
 
-__device__ __forceinline__ void write_partial(Tri *warp_acc, const Tri &acc, double K, double per_value, Tri *__restrict__ out)
+__device__ __forceinline__ void write_partial(Tri *warp_acc, const Tri &acc, double K, double per_value, Tri *__restrict__ out, bool per_lane = false)
 {
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    if (lane == 0) warp_acc[wid] = acc;
+    Tri wa = acc;
+    if (per_lane) warp_merge_ragged(wa, lane);                 // every lane holds an accumulator: fold them first (fixed order)
+    if (lane == 0) warp_acc[wid] = wa;
     __syncthreads();
     if (tid == 0) {
         Tri a = warp_acc[0];
@@ -241,13 +256,20 @@ __device__ __forceinline__ void load16(const float *sm, int pos, float (&v)[ST_R
 
 // One tile of stats_partial_win.  FAST = interior tile of a 16-byte aligned row: all 4096 samples, the whole halo and all
 // 4096 windows exist, so every run is full and nothing needs masking (63 of 64 tiles of a 262144-sample row).
+//
+// First window of a thread, B(own) with own = 16 tid: the window [own, own + nmax) is q = nmax / 16 whole thread runs
+// (runs tid .. tid + q - 1; run r = positions [16 r, 16 r + 16)) plus the first rem = nmax % 16 values of run tid + q.  The
+// run totals are by-products: the tile's own 256 runs give theirs to eq. 1 anyway (T of chan_run16), the q - 1 halo runs
+// that are needed whole are summed by the first q - 1 threads.  One exclusive scan over those <= 511 run totals, Q[r] =
+// sum of runs 0 .. r-1 of y = x - K, gives B(own) = Q[tid + q] - Q[tid] (+ the rem values): no per-sample prefix sums.
 template <bool FAST>
-__device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__restrict__ Ps, float (*wtot)[ST_THREADS / 32],
-                                         int64_t t0, int64_t n_t, int64_t nwin, int nmax, int span, int span4, int nparts, float K,
-                                         Tri &acc, Tri &accb)
+__device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__restrict__ Q, float (*wtot)[ST_THREADS / 32],
+                                         int64_t t0, int64_t n_t, int64_t nwin, int nmax, float K, Tri &acc, Tri &accb)
 {
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int own = ST_RUN * tid;                              // first position of this thread inside the tile
+    const int q = nmax >> 4, rem = nmax & 15;
+    const int nh = q > 0 ? q - 1 : 0;                          // halo runs needed whole: runs 256 .. 256 + nh - 1
     float xo[ST_RUN];
     load16(xs, own, xo);
     int cnt = ST_RUN, wcnt = ST_RUN;
@@ -257,77 +279,76 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
         wcnt = wleft >= ST_RUN ? ST_RUN : (wleft > 0 ? (int)wleft : 0);  // full windows that start there
     }
 
-    // ---- sample statistics (the tile's own 4096 positions) ----
+    // ---- sample statistics (the tile's own 4096 positions); rt = total of the thread's run of y = x - K ----
     float y[ST_RUN];
 #pragma unroll
-    for (int k = 0; k < ST_RUN; ++k) y[k] = xo[k] - K;
-    if (FAST || __all_sync(0xffffffffu, cnt == ST_RUN)) {
+    for (int k = 0; k < ST_RUN; ++k) y[k] = (FAST || k < cnt) ? xo[k] - K : 0.f;
+    float rt;
+    if (FAST || cnt == ST_RUN) {
         float T, S;
         chan_run16(y, T, S);
-        warp_merge_full(T, S);
-        if (lane == 0) tri_merge_chunk(acc, T, S);
+        rt = T;
+        tri_merge_run(acc, T, S);
     } else {
         Tri t = chan_run_ragged(y, cnt);
-        warp_merge_ragged(t, lane);
-        if (lane == 0) tri_merge(acc, t);
+        rt = (float)t.T;
+        tri_merge(acc, t);
     }
 
-    // ---- exclusive prefix sums of x - K over tile + halo (positions past the row end hold x = 0 and are not used;
-    //      FAST: positions past the staged span hold stale finite-or-not values that only reach prefix entries nobody reads) ----
-    float carry = 0.f;
-    for (int part = 0; part < nparts; ++part) {
-        const int pos = part * ST_CHUNK + own;
-        const bool act = pos < span + ST_RUN;                  // this thread's 16 positions start inside the staged span (+1 group for P[span])
-        const bool wact = part == 0 || (pos - ST_RUN * lane) < span + ST_RUN;   // warp-uniform: any lane of this warp active
-        if (!wact) { __syncthreads(); continue; }              // a warp past the staged span has nothing to add (nor in any later part)
-        float v[ST_RUN];
-        float inc = 0.f;
-        if (wact) {
-            if (part == 0) {
+    // ---- exclusive scan of the run totals: the tile's 256 runs, then the nh halo runs (thread tid sums halo run tid) ----
+    const bool hwarp = 32 * wid < nh + 1;                      // warp-uniform: this warp holds halo runs (or the entry after the last)
+    float ht = 0.f;
+    if (tid < nh) {
+        float h[ST_RUN];
+        load16(xs, ST_CHUNK + own, h);
 #pragma unroll
-                for (int k = 0; k < ST_RUN; ++k) v[k] = y[k];
-            } else if (act && pos < span4) {
-                load16(xs, pos, v);
+        for (int k = 0; k < ST_RUN; ++k) ht += (FAST || t0 + ST_CHUNK + own + k < n_t) ? h[k] - K : 0.f;
+    }
+    float inc = rt, inch = ht;
 #pragma unroll
-                for (int k = 0; k < ST_RUN; ++k) v[k] = (FAST || pos + k < span) ? v[k] - K : 0.f;
-            } else {
+    for (int d = 1; d < 32; d <<= 1) {
+        const float o = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += o;
+    }
+    if (hwarp) {
 #pragma unroll
-                for (int k = 0; k < ST_RUN; ++k) v[k] = 0.f;
-            }
-#pragma unroll
-            for (int k = 1; k < ST_RUN; ++k) v[k] += v[k - 1];
-            inc = v[ST_RUN - 1];
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { const float o = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += o; }
-        } else {
-#pragma unroll
-            for (int k = 0; k < ST_RUN; ++k) v[k] = 0.f;
+        for (int d = 1; d < 32; d <<= 1) {
+            const float o = __shfl_up_sync(0xffffffffu, inch, d);
+            if (lane >= d) inch += o;
         }
-        if (lane == 31) wtot[part & 1][wid] = inc;
-        __syncthreads();
-        float off = inc - v[ST_RUN - 1] + carry;
-        {   // exclusive scan of the 8 warp totals by the first 8 lanes of every warp (3 shuffle steps), then two broadcasts
-            float t = wtot[part & 1][lane & 7];
+    }
+    if (lane == 31) { wtot[0][wid] = inc; wtot[1][wid] = inch; }
+    __syncthreads();
+    float below = 0.f, belowh = 0.f, total = 0.f;
+    {
+        const float4 a0 = *reinterpret_cast<const float4 *>(&wtot[0][0]), a1 = *reinterpret_cast<const float4 *>(&wtot[0][4]);
+        const float w[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
 #pragma unroll
-            for (int d = 1; d < 8; d <<= 1) { const float o = __shfl_up_sync(0xffffffffu, t, d); if ((lane & 7) >= d) t += o; }
-            const float below = __shfl_sync(0xffffffffu, t, (wid + 7) & 7);      // inclusive total of warps 0..wid-1 (lane wid-1)
-            if (wid > 0) off += below;
-            carry += __shfl_sync(0xffffffffu, t, 7);
-        }
-        if (act) {
-            float4 *dp = reinterpret_cast<float4 *>(Ps + st_pad(pos));      // E[pos + k] = off + v[k-1]
-            dp[0] = make_float4(off, off + v[0], off + v[1], off + v[2]);
-            dp[1] = make_float4(off + v[3], off + v[4], off + v[5], off + v[6]);
-            dp[2] = make_float4(off + v[7], off + v[8], off + v[9], off + v[10]);
-            dp[3] = make_float4(off + v[11], off + v[12], off + v[13], off + v[14]);
-        }
+        for (int k = 0; k < 8; ++k) { if (k < wid) below += w[k]; total += w[k]; }
+    }
+    const float q_own = below + (inc - rt);                    // Q[tid]
+    Q[tid] = q_own;
+    if (hwarp) {
+        const float4 a0 = *reinterpret_cast<const float4 *>(&wtot[1][0]), a1 = *reinterpret_cast<const float4 *>(&wtot[1][4]);
+        const float w[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+#pragma unroll
+        for (int k = 0; k < 8; ++k) if (k < wid) belowh += w[k];
+        if (tid <= nh) Q[ST_THREADS + tid] = total + belowh + (inch - ht);
     }
     __syncthreads();
 
     // ---- the 16 windows that start at the thread's positions ----
     float b[ST_RUN];
     if (FAST || wcnt > 0) {
-        b[0] = Ps[st_pad(own + nmax)] - Ps[st_pad(own)];
+        b[0] = Q[tid + q] - q_own;
+        if (rem) {                                             // the first rem values of run tid + q
+            float p[ST_RUN];
+            load16(xs, own + 16 * q, p);
+            float ps = 0.f;
+#pragma unroll
+            for (int k = 0; k < ST_RUN - 1; ++k) ps += (k < rem) ? p[k] - K : 0.f;
+            b[0] += ps;
+        }
         if ((nmax & 3) == 0) {                                 // the entering samples x[own + nmax + k] as four 16-byte loads
             float e[ST_RUN];
             load16(xs, own + nmax, e);
@@ -338,17 +359,19 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
             for (int k = 1; k < ST_RUN; ++k) b[k] = b[k - 1] + (xs[st_pad(own + nmax + k - 1)] - xo[k - 1]);
         }
     }
-    if (FAST || __all_sync(0xffffffffu, wcnt == ST_RUN)) {
+    if (FAST || wcnt == ST_RUN) {
         float T, S;
         chan_run16(b, T, S);
-        warp_merge_full(T, S);
-        if (lane == 0) tri_merge_chunk(accb, T, S);
-    } else if (__any_sync(0xffffffffu, wcnt > 0)) {
+        tri_merge_run(accb, T, S);
+    } else if (wcnt > 0) {
         Tri t = chan_run_ragged(b, wcnt);
-        warp_merge_ragged(t, lane);
-        if (lane == 0) tri_merge(accb, t);
+        tri_merge(accb, t);
     }
 }
+
+// dynamic shared memory of stats_partial_win: two landing buffers and the run-total prefix Q[2 * 256 + 1]
+__host__ __device__ inline int st_win_xs_len(int nmax) { return st_pad(((ST_CHUNK + nmax - 1 + 3) & ~3) + ST_RUN); }
+static size_t st_win_smem(int nmax) { return (size_t)(2 * st_win_xs_len(nmax) + 2 * ST_THREADS + 4) * sizeof(float); }
 
 __global__ void __launch_bounds__(ST_THREADS, 3)
 stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax,
@@ -364,13 +387,12 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
     const int tid = threadIdx.x;
     const int span = ST_CHUNK + nmax - 1;                      // samples staged per tile
     const int span4 = (span + 3) & ~3;
-    const int xs_len = st_pad(span4 + ST_RUN);
+    const int xs_len = st_win_xs_len(nmax);
     float *xs0 = reinterpret_cast<float *>(st_smem);           // two landing buffers [st_pad(span4 + 16)]: raw samples, 0 past the row end
-    float *Ps = xs0 + 2 * xs_len;                              // [st_pad(span4 + 32)] exclusive prefix sums of x - K
+    float *Q = xs0 + 2 * xs_len;                               // [2 * 256 + 1] exclusive prefix of the run totals of x - K
     const int64_t nwin = n_t - nmax + 1;                       // full windows per row
     const int64_t tpr = (n_t + ST_CHUNK - 1) / ST_CHUNK;
     const int64_t total = n_dm * tpr;
-    const int nparts = (span + ST_CHUNK - 1) / ST_CHUNK;       // 2 for nmax >= 2
     Tri acc = {0.0, 0.0, 0.0}, accb = {0.0, 0.0, 0.0};
     float K = 0.f;
     bool have_K = false;
@@ -388,19 +410,24 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
     auto interior = [&](const Pos &p) {                        // whole tile + halo inside a 16-byte aligned row
         return ((reinterpret_cast<uintptr_t>(x + p.row * row_stride) & 15) == 0) && ((int64_t)p.tr * ST_CHUNK + span4 <= n_t);
     };
-    // stage a tile into landing buffer `buf` (asynchronous 16-byte copies; scalar loads at the row end / for unaligned rows)
+    // stage a tile into landing buffer `buf` (asynchronous 16-byte copies; scalar loads at the row end / for unaligned rows).
+    // Copy i of a thread moves floats [4 (tid + 256 i), + 4): 1024 floats further in global memory and, with one pad float4
+    // per 16 floats, 1280 further in shared memory, so the loop is two pointer increments and the copy.
+    const int n16 = span4 >> 2;
+    const int dst_tid = st_pad(4 * tid);
     auto stage = [&](const Pos &p, int buf) {
         const int64_t row = p.row, t0 = (int64_t)p.tr * ST_CHUNK;
         const float *rp = x + row * row_stride;
         float *xb = xs0 + buf * xs_len;
         if (interior(p)) {
-            const float *src = rp + t0;
-            for (int p = tid; p < span4 / 4; p += ST_THREADS) cp_async16_st(xb + st_pad(4 * p), src + 4 * p);
+            const float *src = rp + t0 + 4 * tid;
+            float *dst = xb + dst_tid;
+            for (int c = tid; c < n16; c += ST_THREADS, src += 4 * ST_THREADS, dst += 5 * ST_THREADS) cp_async16_st(dst, src);
         } else {
             const bool vec = ((reinterpret_cast<uintptr_t>(rp) & 15) == 0);
-            for (int p = tid; p < span4 / 4; p += ST_THREADS) {
-                const int64_t pos = t0 + 4 * p;
-                float *dst = xb + st_pad(4 * p);
+            for (int c = tid; c < n16; c += ST_THREADS) {
+                const int64_t pos = t0 + 4 * c;
+                float *dst = xb + st_pad(4 * c);
                 if (vec && pos + 3 < n_t) cp_async16_st(dst, rp + pos);
                 else {
 #pragma unroll
@@ -420,7 +447,7 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
         pos = advance(pos);
         const float *xs = xs0 + buf * xs_len;
         asm volatile("cp.async.wait_group 0;" ::: "memory");
-        __syncthreads();                                       // this tile has landed; everyone is done with the previous tile (other buffer, Ps)
+        __syncthreads();                                       // this tile has landed; everyone is done with the previous tile (other buffer, Q)
         if (c + gridDim.x < total) stage(pos, buf ^ 1);        // the next tile streams in while this one is reduced
 
         if (!have_K) {                                         // shift of this CTA: the mean of its first tile
@@ -433,11 +460,11 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
             K = cta_mean(s, (float)cnt, red);
             have_K = true;
         }
-        if (interior(cur)) win_tile<true>(xs, Ps, wtot, t0, n_t, nwin, nmax, span, span4, nparts, K, acc, accb);
-        else win_tile<false>(xs, Ps, wtot, t0, n_t, nwin, nmax, span, span4, nparts, K, acc, accb);
+        if (interior(cur)) win_tile<true>(xs, Q, wtot, t0, n_t, nwin, nmax, K, acc, accb);
+        else win_tile<false>(xs, Q, wtot, t0, n_t, nwin, nmax, K, acc, accb);
     }
-    write_partial(warp_acc, acc, (double)K, 1.0, part_x + blockIdx.x);
-    write_partial(warp_acc, accb, (double)K, (double)nmax, part_b + blockIdx.x);
+    write_partial(warp_acc, acc, (double)K, 1.0, part_x + blockIdx.x, true);
+    write_partial(warp_acc, accb, (double)K, (double)nmax, part_b + blockIdx.x, true);
 }
 
 // ---- kernel 2: merge the block partials (eq. 2, fp64, fixed order) and write the result -----------------
@@ -518,7 +545,7 @@ static cudaError_t stats_win_limit()
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64 || !limit_set[dev]) {
-        e = cudaFuncSetAttribute(stats_partial_win, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(3 * st_pad(ST_CHUNK + 4096 + 2 * ST_RUN) * sizeof(float)));
+        e = cudaFuncSetAttribute(stats_partial_win, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)st_win_smem(4096));
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) limit_set[dev] = true;
     }
@@ -533,8 +560,7 @@ cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
     if (nmax_for_sigma > 0) {
         const int64_t tiles = n_dm * ((n_t + ST_CHUNK - 1) / ST_CHUNK);
         gx = gb = (int)(tiles < ST_GRID ? tiles : ST_GRID);
-        const int span4 = (ST_CHUNK + nmax_for_sigma - 1 + 3) & ~3;
-        const size_t smem = (size_t)(2 * st_pad(span4 + ST_RUN) + st_pad(span4 + 2 * ST_RUN)) * sizeof(float);
+        const size_t smem = st_win_smem(nmax_for_sigma);
         cudaError_t e = stats_win_limit();
         if (e != cudaSuccess) return e;
         stats_partial_win<<<gx, ST_THREADS, smem, s>>>(x, n_dm, n_t, row_stride, nmax_for_sigma, px, pb);
@@ -563,8 +589,7 @@ cudaError_t launch_stats_rows(const float *x, int64_t n_dm, int64_t n_t, int64_t
     size_t smem = 0;
     if (nmax_for_sigma > 0) {
         if ((e = stats_win_limit()) != cudaSuccess) return e;
-        const int span4 = (ST_CHUNK + nmax_for_sigma - 1 + 3) & ~3;
-        smem = (size_t)(2 * st_pad(span4 + ST_RUN) + st_pad(span4 + 2 * ST_RUN)) * sizeof(float);
+        smem = st_win_smem(nmax_for_sigma);
     }
     for (int64_t r0 = 0; r0 < n_dm; r0 += 65535) {               // grid.y limit
         const unsigned ny = (unsigned)(n_dm - r0 < 65535 ? n_dm - r0 : 65535);
