@@ -90,19 +90,6 @@ __device__ __forceinline__ void tri_merge_chunk(Tri &a, float T, float S)
     a.m += n;
 }
 
-// eq. 2 for a lane's own accumulator (+) one FULL 16-value run of the same lane (stats_partial_win: every lane keeps its
-// accumulator in fp64 across tiles, so a tile needs no shuffles; the lanes are merged once, when the CTA writes its partial)
-__device__ __forceinline__ void tri_merge_run(Tri &a, float T, float S)
-{
-    const double n = (double)ST_RUN;
-    if (a.m == 0.0) { a.m = n; a.T = (double)T; a.S = (double)S; return; }
-    const double d = n * a.T - a.m * (double)T;
-    const float rf = __frcp_rn((float)a.m * (float)(a.m + n));          // m (m + n) <= 2^24 * 16 stays well inside fp32's range
-    a.S = a.S + (double)S + d * d * ((double)rf * (1.0 / (double)ST_RUN));
-    a.T += (double)T;
-    a.m += n;
-}
-
 // runs of any length (ragged chunk): eq. 2 in fp64, the left operand always being the lower lanes
 __device__ __forceinline__ void warp_merge_ragged(Tri &t, int lane)
 {
@@ -254,6 +241,50 @@ __device__ __forceinline__ void load16(const float *sm, int pos, float (&v)[ST_R
     }
 }
 
+// What one lane of stats_partial_win carries from tile to tile (the lanes are merged once, when the CTA writes its partials):
+//   samples : the Chan partial of its runs (eq. 1 per 16-value run, eq. 2 between runs), fp32 for up to 32 runs = 512 values
+//             (m32, T32, S32), folded into the fp64 partial `acc` every 32 tiles -- the precision rule of reading A4;
+//   windows : the sums of b and b^2 of its windows about the shift (b = window sum of x - K, so its mean is nmax (mu - K),
+//             small against its spread), fp32 over the 16 windows of a tile, fp64 across tiles.  The paper prescribes no
+//             method for sigma_Nmax; S_b = sum b^2 - (sum b)^2 / n is formed in fp64 when the lane's partial is
+//             written, and everything above a lane is eq. 2 again.
+struct LaneAcc {
+    float m32, T32, S32;
+    Tri acc;
+    double sb, sb2, nb;
+    __device__ __forceinline__ void init() { m32 = 0.f; T32 = 0.f; S32 = 0.f; acc = Tri{0.0, 0.0, 0.0}; sb = 0.0; sb2 = 0.0; nb = 0.0; }
+    // eq. 2: (m32, T32, S32) (+) one full run (16, T, S)
+    __device__ __forceinline__ void push_run(float T, float S)
+    {
+        if (m32 == 0.f) { m32 = (float)ST_RUN; T32 = T; S32 = S; return; }
+        const float d = fmaf((float)ST_RUN, T32, -m32 * T);
+        const float rf = __frcp_rn(m32 * (m32 + (float)ST_RUN)) * (1.0f / (float)ST_RUN);
+        S32 = fmaf(d * d, rf, S32 + S);
+        T32 += T;
+        m32 += (float)ST_RUN;
+        if (m32 == 512.f) { tri_merge_chunk(acc, T32, S32); m32 = 0.f; }
+    }
+    __device__ __forceinline__ void flush()                     // fold a pending fp32 partial (fewer than 32 runs) into acc
+    {
+        if (m32 > 0.f) { const Tri t = {(double)m32, (double)T32, (double)S32}; tri_merge(acc, t); m32 = 0.f; }
+    }
+    __device__ __forceinline__ Tri windows() const
+    {
+        Tri t = {nb, sb, 0.0};
+        if (nb > 0.0) { t.S = sb2 - sb * sb / nb; if (t.S < 0.0) t.S = 0.0; }
+        return t;
+    }
+};
+
+// inclusive warp scan: the shuffle's own predicate (source lane exists) guards the add
+__device__ __forceinline__ float warp_scan_incl(float v)
+{
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1)
+        asm volatile("{.reg .pred p; .reg .f32 t; shfl.sync.up.b32 t|p, %0, %1, 0, 0xffffffff; @p add.f32 %0, %0, t;}" : "+f"(v) : "r"(d));
+    return v;
+}
+
 // One tile of stats_partial_win.  FAST = interior tile of a 16-byte aligned row: all 4096 samples, the whole halo and all
 // 4096 windows exist, so every run is full and nothing needs masking (63 of 64 tiles of a 262144-sample row).
 //
@@ -262,9 +293,10 @@ __device__ __forceinline__ void load16(const float *sm, int pos, float (&v)[ST_R
 // run totals are by-products: the tile's own 256 runs give theirs to eq. 1 anyway (T of chan_run16), the q - 1 halo runs
 // that are needed whole are summed by the first q - 1 threads.  One exclusive scan over those <= 511 run totals, Q[r] =
 // sum of runs 0 .. r-1 of y = x - K, gives B(own) = Q[tid + q] - Q[tid] (+ the rem values): no per-sample prefix sums.
+// The other 15 windows slide: B(t + 1) = B(t) + x[t + nmax] - x[t].
 template <bool FAST>
 __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__restrict__ Q, float (*wtot)[ST_THREADS / 32],
-                                         int64_t t0, int64_t n_t, int64_t nwin, int nmax, float K, Tri &acc, Tri &accb)
+                                         int64_t t0, int64_t n_t, int64_t nwin, int nmax, float K, LaneAcc &L)
 {
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int own = ST_RUN * tid;                              // first position of this thread inside the tile
@@ -280,19 +312,22 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
     }
 
     // ---- sample statistics (the tile's own 4096 positions); rt = total of the thread's run of y = x - K ----
-    float y[ST_RUN];
-#pragma unroll
-    for (int k = 0; k < ST_RUN; ++k) y[k] = (FAST || k < cnt) ? xo[k] - K : 0.f;
     float rt;
-    if (FAST || cnt == ST_RUN) {
-        float T, S;
-        chan_run16(y, T, S);
-        rt = T;
-        tri_merge_run(acc, T, S);
-    } else {
-        Tri t = chan_run_ragged(y, cnt);
-        rt = (float)t.T;
-        tri_merge(acc, t);
+    {
+        float y[ST_RUN];
+#pragma unroll
+        for (int k = 0; k < ST_RUN; ++k) y[k] = (FAST || k < cnt) ? xo[k] - K : 0.f;
+        if (FAST || cnt == ST_RUN) {
+            float T, S;
+            chan_run16(y, T, S);
+            rt = T;
+            L.push_run(T, S);
+        } else {
+            const Tri t = chan_run_ragged(y, cnt);
+            rt = (float)t.T;
+            L.flush();
+            tri_merge(L.acc, t);
+        }
     }
 
     // ---- exclusive scan of the run totals: the tile's 256 runs, then the nh halo runs (thread tid sums halo run tid) ----
@@ -304,19 +339,9 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
 #pragma unroll
         for (int k = 0; k < ST_RUN; ++k) ht += (FAST || t0 + ST_CHUNK + own + k < n_t) ? h[k] - K : 0.f;
     }
-    float inc = rt, inch = ht;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const float o = __shfl_up_sync(0xffffffffu, inc, d);
-        if (lane >= d) inc += o;
-    }
-    if (hwarp) {
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const float o = __shfl_up_sync(0xffffffffu, inch, d);
-            if (lane >= d) inch += o;
-        }
-    }
+    const float inc = warp_scan_incl(rt);
+    float inch = ht;
+    if (hwarp) inch = warp_scan_incl(ht);
     if (lane == 31) { wtot[0][wid] = inc; wtot[1][wid] = inch; }
     __syncthreads();
     float below = 0.f, belowh = 0.f, total = 0.f;
@@ -337,35 +362,34 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
     }
     __syncthreads();
 
-    // ---- the 16 windows that start at the thread's positions ----
-    float b[ST_RUN];
+    // ---- the 16 windows that start at the thread's positions: sums of b and b^2 ----
     if (FAST || wcnt > 0) {
-        b[0] = Q[tid + q] - q_own;
+        float b = Q[tid + q] - q_own;
         if (rem) {                                             // the first rem values of run tid + q
             float p[ST_RUN];
             load16(xs, own + 16 * q, p);
             float ps = 0.f;
 #pragma unroll
             for (int k = 0; k < ST_RUN - 1; ++k) ps += (k < rem) ? p[k] - K : 0.f;
-            b[0] += ps;
+            b += ps;
         }
+        float sb = b, sb2 = b * b;
         if ((nmax & 3) == 0) {                                 // the entering samples x[own + nmax + k] as four 16-byte loads
             float e[ST_RUN];
             load16(xs, own + nmax, e);
 #pragma unroll
-            for (int k = 1; k < ST_RUN; ++k) b[k] = b[k - 1] + (e[k - 1] - xo[k - 1]);
+            for (int k = 1; k < ST_RUN; ++k) {
+                b += e[k - 1] - xo[k - 1];
+                if (FAST || k < wcnt) { sb += b; sb2 = fmaf(b, b, sb2); }
+            }
         } else {
 #pragma unroll
-            for (int k = 1; k < ST_RUN; ++k) b[k] = b[k - 1] + (xs[st_pad(own + nmax + k - 1)] - xo[k - 1]);
+            for (int k = 1; k < ST_RUN; ++k) {
+                b += xs[st_pad(own + nmax + k - 1)] - xo[k - 1];
+                if (FAST || k < wcnt) { sb += b; sb2 = fmaf(b, b, sb2); }
+            }
         }
-    }
-    if (FAST || wcnt == ST_RUN) {
-        float T, S;
-        chan_run16(b, T, S);
-        tri_merge_run(accb, T, S);
-    } else if (wcnt > 0) {
-        Tri t = chan_run_ragged(b, wcnt);
-        tri_merge(accb, t);
+        L.sb += (double)sb; L.sb2 += (double)sb2; L.nb += (double)wcnt;
     }
 }
 
@@ -393,33 +417,34 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
     const int64_t nwin = n_t - nmax + 1;                       // full windows per row
     const int64_t tpr = (n_t + ST_CHUNK - 1) / ST_CHUNK;
     const int64_t total = n_dm * tpr;
-    Tri acc = {0.0, 0.0, 0.0}, accb = {0.0, 0.0, 0.0};
+    LaneAcc L;
+    L.init();
     float K = 0.f;
     bool have_K = false;
 
-    // (row, tile-in-row) of the persistent walk, advanced by the grid size with 32-bit arithmetic (a 64-bit division per
-    // tile costs more instructions than the tile's arithmetic)
+    // (row, tile-in-row) of the persistent walk: the grid size is split once into whole rows and a remainder, so a step
+    // is two adds and a wrap (a division per tile costs more instructions than a third of the tile's arithmetic)
     struct Pos { int64_t row; unsigned tr; };
     const unsigned utpr = (unsigned)tpr;
+    const unsigned step_rows = gridDim.x / utpr, step_tiles = gridDim.x % utpr;
     auto advance = [&](Pos p) {
-        unsigned t = p.tr + gridDim.x;
-        if (t >= utpr) { const unsigned q = t / utpr; p.row += q; t -= q * utpr; }
-        p.tr = t;
+        p.tr += step_tiles; p.row += step_rows;
+        if (p.tr >= utpr) { p.tr -= utpr; ++p.row; }
         return p;
     };
-    auto interior = [&](const Pos &p) {                        // whole tile + halo inside a 16-byte aligned row
-        return ((reinterpret_cast<uintptr_t>(x + p.row * row_stride) & 15) == 0) && ((int64_t)p.tr * ST_CHUNK + span4 <= n_t);
-    };
+    // interior tile: whole tile + halo inside the row, and every row 16-byte aligned (else all tiles take the general path)
+    const bool rows_aligned = ((reinterpret_cast<uintptr_t>(x) & 15) == 0) && ((row_stride & 3) == 0 || n_dm == 1);
+    const unsigned tr_interior = (rows_aligned && n_t >= span4) ? (unsigned)((n_t - span4) / ST_CHUNK + 1) : 0u;   // tiles tr < this
     // stage a tile into landing buffer `buf` (asynchronous 16-byte copies; scalar loads at the row end / for unaligned rows).
     // Copy i of a thread moves floats [4 (tid + 256 i), + 4): 1024 floats further in global memory and, with one pad float4
     // per 16 floats, 1280 further in shared memory, so the loop is two pointer increments and the copy.
     const int n16 = span4 >> 2;
     const int dst_tid = st_pad(4 * tid);
     auto stage = [&](const Pos &p, int buf) {
-        const int64_t row = p.row, t0 = (int64_t)p.tr * ST_CHUNK;
-        const float *rp = x + row * row_stride;
+        const int64_t t0 = (int64_t)p.tr * ST_CHUNK;
+        const float *rp = x + p.row * row_stride;
         float *xb = xs0 + buf * xs_len;
-        if (interior(p)) {
+        if (p.tr < tr_interior) {
             const float *src = rp + t0 + 4 * tid;
             float *dst = xb + dst_tid;
             for (int c = tid; c < n16; c += ST_THREADS, src += 4 * ST_THREADS, dst += 5 * ST_THREADS) cp_async16_st(dst, src);
@@ -460,11 +485,12 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
             K = cta_mean(s, (float)cnt, red);
             have_K = true;
         }
-        if (interior(cur)) win_tile<true>(xs, Q, wtot, t0, n_t, nwin, nmax, K, acc, accb);
-        else win_tile<false>(xs, Q, wtot, t0, n_t, nwin, nmax, K, acc, accb);
+        if (cur.tr < tr_interior) win_tile<true>(xs, Q, wtot, t0, n_t, nwin, nmax, K, L);
+        else win_tile<false>(xs, Q, wtot, t0, n_t, nwin, nmax, K, L);
     }
-    write_partial(warp_acc, acc, (double)K, 1.0, part_x + blockIdx.x, true);
-    write_partial(warp_acc, accb, (double)K, (double)nmax, part_b + blockIdx.x, true);
+    L.flush();
+    write_partial(warp_acc, L.acc, (double)K, 1.0, part_x + blockIdx.x, true);
+    write_partial(warp_acc, L.windows(), (double)K, (double)nmax, part_b + blockIdx.x, true);
 }
 
 // ---- kernel 2: merge the block partials (eq. 2, fp64, fixed order) and write the result -----------------
