@@ -7,9 +7,11 @@
 // accumulator.  Each CTA writes one (m, T, S) partial.  Two variants:
 //   stats_partial      (nmax_for_sigma = 0): 16-byte streaming loads straight into registers.
 //   stats_partial_win  (nmax_for_sigma > 0): the chunk and its nmax-1 halo samples are staged in shared memory ONCE;
-//                      the same data gives the sample statistics and the Nmax-sample boxcar SUMS of every full window
-//                      (first window of a thread from a tile-local fp32 prefix scan, the next 15 slide), which go
-//                      through the same eq. 1 / eq. 2 reduction.  x is read once (plus the halo, which hits L2).
+//                      the same data gives the sample statistics (eq. 1 per 16-sample run, eq. 2 into a per-lane partial
+//                      that lives across tiles) and the Nmax-sample boxcar SUMS of every full window: the first window
+//                      of a thread from an exclusive scan over the 16-sample RUN TOTALS of the tile (by-products of
+//                      eq. 1), the next 15 by sliding; their statistics are sums of b and b^2 about the shift (the paper
+//                      prescribes no method for sigma_Nmax).  x is read once (plus the halo, which hits L2).
 // Kernel 2 (stats_finalize) merges the partials with eq. 2 in index order (fp64, fixed order => bit-reproducible) and
 // writes mu = T/n, sigma = sqrt(S/n), sigma_nmax.
 //
@@ -20,6 +22,8 @@
 //
 // Roofline: pure HBM stream, 4 B/sample read.
 #include "spd_common.cuh"
+
+#include <mutex>
 
 namespace spd {
 
@@ -285,6 +289,33 @@ __device__ __forceinline__ float warp_scan_incl(float v)
     return v;
 }
 
+// both scans of a halo warp, level by level (two independent chains)
+__device__ __forceinline__ void warp_scan_incl2(float &a, float &b)
+{
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1)
+        asm volatile("{.reg .pred p; .reg .f32 t, u; shfl.sync.up.b32 t|p, %0, %2, 0, 0xffffffff; shfl.sync.up.b32 u, %1, %2, 0, 0xffffffff;\n\t"
+                     "@p add.f32 %0, %0, t; @p add.f32 %1, %1, u;}" : "+f"(a), "+f"(b) : "r"(d));
+}
+
+// split CTA barrier: an mbarrier in shared memory; arrive does not wait, wait spins on the phase parity (acquire)
+__device__ __forceinline__ void mbar_init(unsigned long long *b, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"((unsigned)__cvta_generic_to_shared(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *b)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"((unsigned)__cvta_generic_to_shared(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity)
+{
+    unsigned ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"((unsigned)__cvta_generic_to_shared(b)), "r"(parity) : "memory");
+    } while (!ok);
+}
+
 // One tile of stats_partial_win.  FAST = interior tile of a 16-byte aligned row: all 4096 samples, the whole halo and all
 // 4096 windows exist, so every run is full and nothing needs masking (63 of 64 tiles of a 262144-sample row).
 //
@@ -296,7 +327,8 @@ __device__ __forceinline__ float warp_scan_incl(float v)
 // The other 15 windows slide: B(t + 1) = B(t) + x[t + nmax] - x[t].
 template <bool FAST>
 __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__restrict__ Q, float (*wtot)[ST_THREADS / 32],
-                                         int64_t t0, int64_t n_t, int64_t nwin, int nmax, float K, LaneAcc &L)
+                                         int64_t t0, int64_t n_t, int64_t nwin, int nmax, float K, LaneAcc &L,
+                                         unsigned long long *mbar, unsigned parity)
 {
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int own = ST_RUN * tid;                              // first position of this thread inside the tile
@@ -311,39 +343,38 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
         wcnt = wleft >= ST_RUN ? ST_RUN : (wleft > 0 ? (int)wleft : 0);  // full windows that start there
     }
 
-    // ---- sample statistics (the tile's own 4096 positions); rt = total of the thread's run of y = x - K ----
-    float rt;
-    {
-        float y[ST_RUN];
+    // ---- run totals first (the other warps wait for them), then the scan; the CTA-wide steps are split barriers
+    //      (arrive ... independent work ... sync), so a warp that is ahead keeps issuing ----
+    float y[ST_RUN];
 #pragma unroll
-        for (int k = 0; k < ST_RUN; ++k) y[k] = (FAST || k < cnt) ? xo[k] - K : 0.f;
-        if (FAST || cnt == ST_RUN) {
-            float T, S;
-            chan_run16(y, T, S);
-            rt = T;
-            L.push_run(T, S);
-        } else {
-            const Tri t = chan_run_ragged(y, cnt);
-            rt = (float)t.T;
-            L.flush();
-            tri_merge(L.acc, t);
-        }
-    }
-
-    // ---- exclusive scan of the run totals: the tile's 256 runs, then the nh halo runs (thread tid sums halo run tid) ----
+    for (int k = 0; k < ST_RUN; ++k) y[k] = (FAST || k < cnt) ? xo[k] - K : 0.f;
+    const float rt = (((y[0] + y[1]) + (y[2] + y[3])) + ((y[4] + y[5]) + (y[6] + y[7]))) +
+                     (((y[8] + y[9]) + (y[10] + y[11])) + ((y[12] + y[13]) + (y[14] + y[15])));
     const bool hwarp = 32 * wid < nh + 1;                      // warp-uniform: this warp holds halo runs (or the entry after the last)
     float ht = 0.f;
-    if (tid < nh) {
+    if (tid < nh) {                                            // thread tid sums halo run tid
         float h[ST_RUN];
         load16(xs, ST_CHUNK + own, h);
 #pragma unroll
         for (int k = 0; k < ST_RUN; ++k) ht += (FAST || t0 + ST_CHUNK + own + k < n_t) ? h[k] - K : 0.f;
     }
-    const float inc = warp_scan_incl(rt);
-    float inch = ht;
-    if (hwarp) inch = warp_scan_incl(ht);
-    if (lane == 31) { wtot[0][wid] = inc; wtot[1][wid] = inch; }
-    __syncthreads();
+    float inc = rt, inch = ht;
+    if (hwarp) warp_scan_incl2(inc, inch); else inc = warp_scan_incl(inc);
+    if (lane == 31) { wtot[0][wid] = inc; wtot[1][wid] = inch; mbar_arrive(mbar); }      // 8 arrivals complete the phase
+
+    // ---- sample statistics of the tile's own 4096 positions (eq. 1 per run, eq. 2 into the lane's partial) ----
+    if (FAST || cnt == ST_RUN) {
+        float T, S;
+        chan_run16(y, T, S);
+        L.push_run(T, S);
+    } else {
+        const Tri t = chan_run_ragged(y, cnt);
+        L.flush();
+        tri_merge(L.acc, t);
+    }
+
+    // ---- exclusive prefix Q of the run totals: the tile's 256 runs, then the nh halo runs ----
+    mbar_wait(mbar, parity);
     float below = 0.f, belowh = 0.f, total = 0.f;
     {
         const float4 a0 = *reinterpret_cast<const float4 *>(&wtot[0][0]), a1 = *reinterpret_cast<const float4 *>(&wtot[0][4]);
@@ -360,34 +391,35 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
         for (int k = 0; k < 8; ++k) if (k < wid) belowh += w[k];
         if (tid <= nh) Q[ST_THREADS + tid] = total + belowh + (inch - ht);
     }
-    __syncthreads();
+    mbar_arrive(mbar + 1);                                     // every thread wrote its Q entries: 256 arrivals
 
-    // ---- the 16 windows that start at the thread's positions: sums of b and b^2 ----
+    // ---- the 16 windows that start at the thread's positions: sums of b and b^2.  de[k] = x[own + nmax + k] - x[own + k] is
+    //      what a slide adds; it needs nothing from other warps, so it is formed before the wait for Q ----
+    float de[ST_RUN - 1];
+    if ((nmax & 3) == 0) {                                     // the entering samples as four 16-byte loads
+        float e[ST_RUN];
+        load16(xs, own + nmax, e);
+#pragma unroll
+        for (int k = 0; k < ST_RUN - 1; ++k) de[k] = e[k] - xo[k];
+    } else {
+#pragma unroll
+        for (int k = 0; k < ST_RUN - 1; ++k) de[k] = xs[st_pad(own + nmax + k)] - xo[k];
+    }
+    float ps = 0.f;
+    if (rem) {                                                 // the first rem values of run tid + q
+        float p[ST_RUN];
+        load16(xs, own + 16 * q, p);
+#pragma unroll
+        for (int k = 0; k < ST_RUN - 1; ++k) ps += (k < rem) ? p[k] - K : 0.f;
+    }
+    mbar_wait(mbar + 1, parity);
     if (FAST || wcnt > 0) {
-        float b = Q[tid + q] - q_own;
-        if (rem) {                                             // the first rem values of run tid + q
-            float p[ST_RUN];
-            load16(xs, own + 16 * q, p);
-            float ps = 0.f;
-#pragma unroll
-            for (int k = 0; k < ST_RUN - 1; ++k) ps += (k < rem) ? p[k] - K : 0.f;
-            b += ps;
-        }
+        float b = (Q[tid + q] - q_own) + ps;
         float sb = b, sb2 = b * b;
-        if ((nmax & 3) == 0) {                                 // the entering samples x[own + nmax + k] as four 16-byte loads
-            float e[ST_RUN];
-            load16(xs, own + nmax, e);
 #pragma unroll
-            for (int k = 1; k < ST_RUN; ++k) {
-                b += e[k - 1] - xo[k - 1];
-                if (FAST || k < wcnt) { sb += b; sb2 = fmaf(b, b, sb2); }
-            }
-        } else {
-#pragma unroll
-            for (int k = 1; k < ST_RUN; ++k) {
-                b += xs[st_pad(own + nmax + k - 1)] - xo[k - 1];
-                if (FAST || k < wcnt) { sb += b; sb2 = fmaf(b, b, sb2); }
-            }
+        for (int k = 1; k < ST_RUN; ++k) {
+            b += de[k - 1];
+            if (FAST || k < wcnt) { sb += b; sb2 = fmaf(b, b, sb2); }
         }
         L.sb += (double)sb; L.sb2 += (double)sb2; L.nb += (double)wcnt;
     }
@@ -408,7 +440,14 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
     __shared__ Tri warp_acc[ST_THREADS / 32];
     __shared__ float red[2 * ST_THREADS / 32];
     __shared__ __align__(16) float wtot[2][ST_THREADS / 32];
+    __shared__ unsigned long long mbar[2];                     // split barriers of a tile: warp totals written (8 arrivals), Q written (256)
     const int tid = threadIdx.x;
+    if (tid == 0) {
+        mbar_init(mbar, ST_THREADS / 32);
+        mbar_init(mbar + 1, ST_THREADS);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    unsigned parity = 0;                                       // phase of both barriers: one phase per tile
     const int span = ST_CHUNK + nmax - 1;                      // samples staged per tile
     const int span4 = (span + 3) & ~3;
     const int xs_len = st_win_xs_len(nmax);
@@ -485,8 +524,9 @@ stats_partial_win(const float *__restrict__ x, int64_t n_dm, int64_t n_t, int64_
             K = cta_mean(s, (float)cnt, red);
             have_K = true;
         }
-        if (cur.tr < tr_interior) win_tile<true>(xs, Q, wtot, t0, n_t, nwin, nmax, K, L);
-        else win_tile<false>(xs, Q, wtot, t0, n_t, nwin, nmax, K, L);
+        if (cur.tr < tr_interior) win_tile<true>(xs, Q, wtot, t0, n_t, nwin, nmax, K, L, mbar, parity);
+        else win_tile<false>(xs, Q, wtot, t0, n_t, nwin, nmax, K, L, mbar, parity);
+        parity ^= 1u;
     }
     L.flush();
     write_partial(warp_acc, L.acc, (double)K, 1.0, part_x + blockIdx.x, true);
@@ -563,18 +603,32 @@ __global__ void stats_merge_kernel(const spd_stats_t *__restrict__ parts, int co
     fill_stats(out, a, b, nm < 0 ? 0 : nm);
 }
 
-// per device: the dynamic shared-memory limit of stats_partial_win, set once to the largest tile (nmax = 4096)
-static cudaError_t stats_win_limit()
+// stats_partial_win runs ONE resident wave of persistent CTAs.  Per device, the dynamic shared-memory limit is set once (to
+// the largest tile, nmax = 4096) and the resident CTAs per SM of a shared-memory size are looked up once (the queries cost
+// tens of microseconds per launch otherwise).
+static cudaError_t stats_win_wave(size_t smem, int *wave)
 {
+    static std::mutex mu;
     static bool limit_set[64] = {};
+    struct Entry { int dev; size_t smem; int wave; };
+    static Entry cache[64];
+    static int n_cached = 0;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lk(mu);
     if (dev < 0 || dev >= 64 || !limit_set[dev]) {
         e = cudaFuncSetAttribute(stats_partial_win, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)st_win_smem(4096));
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) limit_set[dev] = true;
     }
+    for (int i = 0; i < n_cached; ++i) if (cache[i].dev == dev && cache[i].smem == smem) { *wave = cache[i].wave; return cudaSuccess; }
+    int sms = 0, per_sm = 0;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stats_partial_win, ST_THREADS, smem)) != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorInvalidConfiguration;
+    *wave = sms * per_sm < MAX_PARTIALS ? sms * per_sm : MAX_PARTIALS;
+    if (n_cached < 64) cache[n_cached++] = Entry{dev, smem, *wave};
     return cudaSuccess;
 }
 
@@ -585,10 +639,11 @@ cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
     int gx = 0, gb = 0;
     if (nmax_for_sigma > 0) {
         const int64_t tiles = n_dm * ((n_t + ST_CHUNK - 1) / ST_CHUNK);
-        gx = gb = (int)(tiles < ST_GRID ? tiles : ST_GRID);
         const size_t smem = st_win_smem(nmax_for_sigma);
-        cudaError_t e = stats_win_limit();
+        int wave = 0;
+        cudaError_t e = stats_win_wave(smem, &wave);
         if (e != cudaSuccess) return e;
+        gx = gb = (int)(tiles < wave ? tiles : wave);
         stats_partial_win<<<gx, ST_THREADS, smem, s>>>(x, n_dm, n_t, row_stride, nmax_for_sigma, px, pb);
     } else {
         int64_t rows = n_dm, cols = n_t, stride = row_stride;
@@ -614,8 +669,9 @@ cudaError_t launch_stats_rows(const float *x, int64_t n_dm, int64_t n_t, int64_t
     cudaError_t e;
     size_t smem = 0;
     if (nmax_for_sigma > 0) {
-        if ((e = stats_win_limit()) != cudaSuccess) return e;
         smem = st_win_smem(nmax_for_sigma);
+        int wave = 0;
+        if ((e = stats_win_wave(smem, &wave)) != cudaSuccess) return e;
     }
     for (int64_t r0 = 0; r0 < n_dm; r0 += 65535) {               // grid.y limit
         const unsigned ny = (unsigned)(n_dm - r0 < 65535 ? n_dm - r0 : 65535);
