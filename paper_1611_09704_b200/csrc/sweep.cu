@@ -268,6 +268,20 @@ struct Norm {
         v = __fadd2_rn(__fadd2_rn(v, mu_hi2), mu_lo2);
         return RC ? __fmul2_rn(v, rs2) : v;
     }
+    // the same arithmetic for two CONSECUTIVE raw samples (p, q) of one sub-tile, as they sit in the registers of a 16-byte
+    // load: the packed steps run on that native pair and the last step is scalar, so the results can be written straight
+    // into the interleaved (sub-tile A, sub-tile B) pairs without register moves (same issue slots: a packed op takes two)
+    template <bool RC>
+    __device__ __forceinline__ void apply_pair(float p, float q, float &op, float &oq) const
+    {
+        float2 v = __fadd2_rn(make_float2(p, q), mu_hi2);
+        if (RC) {
+            v = __fadd2_rn(v, mu_lo2);
+            op = __fmul_rn(v.x, rs2.x); oq = __fmul_rn(v.y, rs2.x);
+        } else {
+            op = __fadd_rn(v.x, mu_lo2.x); oq = __fadd_rn(v.y, mu_lo2.x);
+        }
+    }
 };
 
 // 8 groups of one raw tile -> 8 interleaved values (sub-tile A, sub-tile B) of group g
@@ -278,6 +292,18 @@ __device__ __forceinline__ void load_group(const float *raw, int g, float2 (&v)[
     const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
     v[0] = make_float2(a0.x, b0.x); v[1] = make_float2(a0.y, b0.y); v[2] = make_float2(a0.z, b0.z); v[3] = make_float2(a0.w, b0.w);
     v[4] = make_float2(a1.x, b1.x); v[5] = make_float2(a1.y, b1.y); v[6] = make_float2(a1.z, b1.z); v[7] = make_float2(a1.w, b1.w);
+}
+
+// the same with y = x - mu (and / sigma) formed on the way (Norm::apply_pair)
+template <int SW_SUB, bool RC>
+__device__ __forceinline__ void load_norm_group(const float *raw, int g, const Norm &norm, float2 (&v)[SW_R])
+{
+    const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
+    const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
+    norm.apply_pair<RC>(a0.x, a0.y, v[0].x, v[1].x); norm.apply_pair<RC>(a0.z, a0.w, v[2].x, v[3].x);
+    norm.apply_pair<RC>(a1.x, a1.y, v[4].x, v[5].x); norm.apply_pair<RC>(a1.z, a1.w, v[6].x, v[7].x);
+    norm.apply_pair<RC>(b0.x, b0.y, v[0].y, v[1].y); norm.apply_pair<RC>(b0.z, b0.w, v[2].y, v[3].y);
+    norm.apply_pair<RC>(b1.x, b1.y, v[4].y, v[5].y); norm.apply_pair<RC>(b1.z, b1.w, v[6].y, v[7].y);
 }
 
 // group g of the working layout: Z[zpad(8 g + j)] = v[j], four 16-byte stores (zpad(8 g) = 10 g)
@@ -760,10 +786,12 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
     const int nblk = sw_nblk(nmax);
     const int H = sw_halo(nmax);
     const int LRAW = SW_TILE + H, LZ = SW_SUB + H;
-    const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
     Norm norm(st);
     const float NINF = __int_as_float(0xff800000);
     const int mask31 = opaque_reg(~31);
+    // every row of both planes 16-byte aligned: whole tiles take the straight-line store path
+    const bool planes_fast = ((reinterpret_cast<uintptr_t>(snr) & 15) == 0) && ((out_stride & 3) == 0) &&
+                             (width == nullptr || (((reinterpret_cast<uintptr_t>(width) & 15) == 0) && ((out_stride & 7) == 0)));
     const bool row_tables = !RC && stats_stride != 0;
 
     if (!RC && !row_tables) for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = __ldg(table + w);
@@ -790,17 +818,16 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
         __syncthreads();                           // raw tile landed; everyone is done with the previous Z
 
         float2 B[SW_R], W[SW_R], best[SW_R], tbest[SW_R];
-        for (int part = 0; part < nparts; ++part) {
-            const int g = part * SW_THREADS + tid;
-            if (8 * g < LZ) {
-                float2 v[SW_R];
-                load_group<SW_SUB>(raw, g, v);
-                if (DEC && dec_out != nullptr && part == 0) {         // the tile's own samples, summed in pairs: the next level's series
+        {   // the thread's own 8 + 8 samples: they stay in registers as the first window
+            if (!DEC) load_norm_group<SW_SUB, RC>(raw, tid, norm, W);
+            else {
+                load_group<SW_SUB>(raw, tid, W);
+                if (dec_out != nullptr) {              // the tile's own samples, summed in pairs: the next level's series
                     const int64_t n_next = n_t >> 1;
                     const int64_t ia = (T0 + SW_R * tid) >> 1, ib = ia + SW_SUB / 2;
                     float *da = dec_out + row * dec_stride + ia, *db = dec_out + row * dec_stride + ib;
-                    const float4 sa = make_float4(__fadd_rn(v[0].x, v[1].x), __fadd_rn(v[2].x, v[3].x), __fadd_rn(v[4].x, v[5].x), __fadd_rn(v[6].x, v[7].x));
-                    const float4 sb = make_float4(__fadd_rn(v[0].y, v[1].y), __fadd_rn(v[2].y, v[3].y), __fadd_rn(v[4].y, v[5].y), __fadd_rn(v[6].y, v[7].y));
+                    const float4 sa = make_float4(__fadd_rn(W[0].x, W[1].x), __fadd_rn(W[2].x, W[3].x), __fadd_rn(W[4].x, W[5].x), __fadd_rn(W[6].x, W[7].x));
+                    const float4 sb = make_float4(__fadd_rn(W[0].y, W[1].y), __fadd_rn(W[2].y, W[3].y), __fadd_rn(W[4].y, W[5].y), __fadd_rn(W[6].y, W[7].y));
                     const bool al = ((reinterpret_cast<uintptr_t>(dec_out + row * dec_stride) & 15) == 0);
                     if (al && ia + 3 < n_next) *reinterpret_cast<float4 *>(da) = sa;
                     else { const float t[4] = {sa.x, sa.y, sa.z, sa.w}; for (int k = 0; k < 4; ++k) if (ia + k < n_next) da[k] = t[k]; }
@@ -808,12 +835,14 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
                     else { const float t[4] = {sb.x, sb.y, sb.z, sb.w}; for (int k = 0; k < 4; ++k) if (ib + k < n_next) db[k] = t[k]; }
                 }
 #pragma unroll
-                for (int j = 0; j < SW_R; ++j) {
-                    v[j] = norm.apply<RC>(v[j]);
-                    if (part == 0) W[j] = v[j];
-                }
-                store_group(Z, g, v);
+                for (int j = 0; j < SW_R; ++j) W[j] = norm.apply<RC>(W[j]);
             }
+            store_group(Z, tid, W);
+        }
+        for (int g = SW_THREADS + tid; 8 * g < LZ; g += SW_THREADS) {      // the halo positions past the sub-tile
+            float2 v[SW_R];
+            load_norm_group<SW_SUB, RC>(raw, g, norm, v);
+            store_group(Z, g, v);
         }
         __syncthreads();                           // Z complete; raw is free again
         if (tile + gridDim.x < total_tiles) stg.stage<SW_THREADS, true>(raw, x, n_t, row_stride, pos, LRAW, tid);
@@ -829,6 +858,28 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
         }
         if (nblk > 2) sweep8_tagged<2, RC, true>(B, W, best, tbest, zp + 20, rtf + 16, mask31);
         if (nblk > 3) sweep8_tagged<3, RC, true>(B, W, best, tbest, zp + 30, rtf + 24, mask31);
+
+        if (!DEC && planes_fast && T0 + SW_TILE <= n_t && (RC || rtf[0] == rtf[0])) {      // (a NaN table must surface: general path)
+            // whole tile inside 16-byte aligned planes (all but the last tile of a row): six 16-byte streaming stores per thread,
+            // and the widths are decoded two at a time, (32 - tag_lo) | (32 - tag_hi) << 16 = 0x00200020 - (tags picked by PRMT)
+            float *oa = snr + row * out_stride + (T0 + SW_R * tid), *ob = oa + SW_SUB;
+            __stcs(reinterpret_cast<float4 *>(oa), make_float4(best[0].x, best[1].x, best[2].x, best[3].x));
+            __stcs(reinterpret_cast<float4 *>(oa) + 1, make_float4(best[4].x, best[5].x, best[6].x, best[7].x));
+            __stcs(reinterpret_cast<float4 *>(ob), make_float4(best[0].y, best[1].y, best[2].y, best[3].y));
+            __stcs(reinterpret_cast<float4 *>(ob) + 1, make_float4(best[4].y, best[5].y, best[6].y, best[7].y));
+            if (width) {
+                uint16_t *wa = width + row * out_stride + (T0 + SW_R * tid), *wb = wa + SW_SUB;
+                unsigned pa[4], pb[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    pa[k] = 0x00200020u - (__byte_perm(__float_as_uint(tbest[2 * k].x), __float_as_uint(tbest[2 * k + 1].x), 0x4400) & 0x001f001fu);
+                    pb[k] = 0x00200020u - (__byte_perm(__float_as_uint(tbest[2 * k].y), __float_as_uint(tbest[2 * k + 1].y), 0x4400) & 0x001f001fu);
+                }
+                __stcs(reinterpret_cast<uint4 *>(wa), make_uint4(pa[0], pa[1], pa[2], pa[3]));
+                __stcs(reinterpret_cast<uint4 *>(wb), make_uint4(pb[0], pb[1], pb[2], pb[3]));
+            }
+            continue;
+        }
 
         int wx[SW_R], wy[SW_R];
 #pragma unroll
