@@ -295,11 +295,15 @@ __device__ __forceinline__ void load_group(const float *raw, int g, float2 (&v)[
 }
 
 // the same with y = x - mu (and / sigma) formed on the way (Norm::apply_pair)
-template <int SW_SUB, bool RC>
-__device__ __forceinline__ void load_norm_group(const float *raw, int g, const Norm &norm, float2 (&v)[SW_R])
+template <int SW_SUB, bool RC, bool PAIRSUMS = false>
+__device__ __forceinline__ void load_norm_group(const float *raw, int g, const Norm &norm, float2 (&v)[SW_R], float4 *sa = nullptr, float4 *sb = nullptr)
 {
     const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
     const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
+    if (PAIRSUMS) {                                   // x'[i] = x[2i] + x[2i+1] of the RAW samples (decimation in time)
+        *sa = make_float4(__fadd_rn(a0.x, a0.y), __fadd_rn(a0.z, a0.w), __fadd_rn(a1.x, a1.y), __fadd_rn(a1.z, a1.w));
+        *sb = make_float4(__fadd_rn(b0.x, b0.y), __fadd_rn(b0.z, b0.w), __fadd_rn(b1.x, b1.y), __fadd_rn(b1.z, b1.w));
+    }
     norm.apply_pair<RC>(a0.x, a0.y, v[0].x, v[1].x); norm.apply_pair<RC>(a0.z, a0.w, v[2].x, v[3].x);
     norm.apply_pair<RC>(a1.x, a1.y, v[4].x, v[5].x); norm.apply_pair<RC>(a1.z, a1.w, v[6].x, v[7].x);
     norm.apply_pair<RC>(b0.x, b0.y, v[0].y, v[1].y); norm.apply_pair<RC>(b0.z, b0.w, v[2].y, v[3].y);
@@ -499,9 +503,7 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
                 float2 *tot = scan + 4 * (part & 1);
                 if (wact) {
                     if (act) {
-                        load_group<SW_SUB>(raw, g, v);
-#pragma unroll
-                        for (int j = 0; j < SW_R; ++j) v[j] = norm.apply<RC>(v[j]);
+                        load_norm_group<SW_SUB, RC>(raw, g, norm, v);
                         store_group(Z, g, v);
                     } else {
 #pragma unroll
@@ -642,7 +644,6 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
     const int nblk = sw_nblk(nmax);
     const int H = sw_halo(nmax);
     const int LRAW = SW_TILE + H, LZ = SW_SUB + H;
-    const int nparts = (LZ + SW_SUB - 1) / SW_SUB;
     Norm norm(st);
     const float NINF = __int_as_float(0xff800000);
     const bool row_tables = !RC && stats_stride != 0;
@@ -674,18 +675,12 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
         __syncthreads();                           // raw tile landed; everyone is done with the previous Z
 
         float2 B[SW_R], W[SW_R], best[SW_R];
-        for (int part = 0; part < nparts; ++part) {
-            const int g = part * SW_THREADS + tid;
-            if (8 * g < LZ) {
-                float2 v[SW_R];
-                load_group<SW_SUB>(raw, g, v);
-#pragma unroll
-                for (int j = 0; j < SW_R; ++j) {
-                    v[j] = norm.apply<RC>(v[j]);
-                    if (part == 0) W[j] = v[j];
-                }
-                store_group(Z, g, v);
-            }
+        load_norm_group<SW_SUB, RC>(raw, tid, norm, W);          // the thread's own 8 + 8 samples stay in registers as the first window
+        store_group(Z, tid, W);
+        for (int g = SW_THREADS + tid; 8 * g < LZ; g += SW_THREADS) {      // the halo positions past the sub-tile
+            float2 v[SW_R];
+            load_norm_group<SW_SUB, RC>(raw, g, norm, v);
+            store_group(Z, g, v);
         }
         __syncthreads();                           // Z complete; raw is free again
         if (tile + gridDim.x < total_tiles) stg.stage<SW_THREADS, false>(raw, x, n_t, row_stride, pos, LRAW, tid);
@@ -819,23 +814,18 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
 
         float2 B[SW_R], W[SW_R], best[SW_R], tbest[SW_R];
         {   // the thread's own 8 + 8 samples: they stay in registers as the first window
-            if (!DEC) load_norm_group<SW_SUB, RC>(raw, tid, norm, W);
-            else {
-                load_group<SW_SUB>(raw, tid, W);
-                if (dec_out != nullptr) {              // the tile's own samples, summed in pairs: the next level's series
-                    const int64_t n_next = n_t >> 1;
-                    const int64_t ia = (T0 + SW_R * tid) >> 1, ib = ia + SW_SUB / 2;
-                    float *da = dec_out + row * dec_stride + ia, *db = dec_out + row * dec_stride + ib;
-                    const float4 sa = make_float4(__fadd_rn(W[0].x, W[1].x), __fadd_rn(W[2].x, W[3].x), __fadd_rn(W[4].x, W[5].x), __fadd_rn(W[6].x, W[7].x));
-                    const float4 sb = make_float4(__fadd_rn(W[0].y, W[1].y), __fadd_rn(W[2].y, W[3].y), __fadd_rn(W[4].y, W[5].y), __fadd_rn(W[6].y, W[7].y));
-                    const bool al = ((reinterpret_cast<uintptr_t>(dec_out + row * dec_stride) & 15) == 0);
-                    if (al && ia + 3 < n_next) *reinterpret_cast<float4 *>(da) = sa;
-                    else { const float t[4] = {sa.x, sa.y, sa.z, sa.w}; for (int k = 0; k < 4; ++k) if (ia + k < n_next) da[k] = t[k]; }
-                    if (al && ib + 3 < n_next) *reinterpret_cast<float4 *>(db) = sb;
-                    else { const float t[4] = {sb.x, sb.y, sb.z, sb.w}; for (int k = 0; k < 4; ++k) if (ib + k < n_next) db[k] = t[k]; }
-                }
-#pragma unroll
-                for (int j = 0; j < SW_R; ++j) W[j] = norm.apply<RC>(W[j]);
+            if (!DEC || dec_out == nullptr) load_norm_group<SW_SUB, RC>(raw, tid, norm, W);
+            else {                                     // ... and, summed in pairs, they are the next level's series
+                float4 sa, sb;
+                load_norm_group<SW_SUB, RC, true>(raw, tid, norm, W, &sa, &sb);
+                const int64_t n_next = n_t >> 1;
+                const int64_t ia = (T0 + SW_R * tid) >> 1, ib = ia + SW_SUB / 2;
+                float *da = dec_out + row * dec_stride + ia, *db = dec_out + row * dec_stride + ib;
+                const bool al = ((reinterpret_cast<uintptr_t>(dec_out + row * dec_stride) & 15) == 0);
+                if (al && ia + 3 < n_next) *reinterpret_cast<float4 *>(da) = sa;
+                else { const float t[4] = {sa.x, sa.y, sa.z, sa.w}; for (int k = 0; k < 4; ++k) if (ia + k < n_next) da[k] = t[k]; }
+                if (al && ib + 3 < n_next) *reinterpret_cast<float4 *>(db) = sb;
+                else { const float t[4] = {sb.x, sb.y, sb.z, sb.w}; for (int k = 0; k < 4; ++k) if (ib + k < n_next) db[k] = t[k]; }
             }
             store_group(Z, tid, W);
         }
@@ -859,7 +849,8 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
         if (nblk > 2) sweep8_tagged<2, RC, true>(B, W, best, tbest, zp + 20, rtf + 16, mask31);
         if (nblk > 3) sweep8_tagged<3, RC, true>(B, W, best, tbest, zp + 30, rtf + 24, mask31);
 
-        if (!DEC && planes_fast && T0 + SW_TILE <= n_t && (RC || rtf[0] == rtf[0])) {      // (a NaN table must surface: general path)
+        if (planes_fast && T0 + SW_TILE + (DEC ? H : 0) <= n_t && (RC || rtf[0] == rtf[0])) {      // (a NaN table must surface: general path;
+                                                               //  a decimated level: every width must fit at every position of the tile)
             // whole tile inside 16-byte aligned planes (all but the last tile of a row): six 16-byte streaming stores per thread,
             // and the widths are decoded two at a time, (32 - tag_lo) | (32 - tag_hi) << 16 = 0x00200020 - (tags picked by PRMT)
             float *oa = snr + row * out_stride + (T0 + SW_R * tid), *ob = oa + SW_SUB;
@@ -874,6 +865,7 @@ boxcar_snr_sweep_narrow(const float *__restrict__ x, int64_t n_t, int64_t row_st
                 for (int k = 0; k < 4; ++k) {
                     pa[k] = 0x00200020u - (__byte_perm(__float_as_uint(tbest[2 * k].x), __float_as_uint(tbest[2 * k + 1].x), 0x4400) & 0x001f001fu);
                     pb[k] = 0x00200020u - (__byte_perm(__float_as_uint(tbest[2 * k].y), __float_as_uint(tbest[2 * k + 1].y), 0x4400) & 0x001f001fu);
+                    if (DEC) { pa[k] *= (unsigned)wscale; pb[k] *= (unsigned)wscale; }       // effective widths w' 2^l <= 4096: no carry between the halves
                 }
                 __stcs(reinterpret_cast<uint4 *>(wa), make_uint4(pa[0], pa[1], pa[2], pa[3]));
                 __stcs(reinterpret_cast<uint4 *>(wb), make_uint4(pb[0], pb[1], pb[2], pb[3]));
