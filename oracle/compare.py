@@ -217,3 +217,83 @@ def compare_candidates(g_dm, g_t, g_snr, g_width, g_count: int, capacity: int,
             r.fail(f"{int(worse.sum())} near-tie candidate widths whose oracle SNR is not within {TIE} of best, first at "
                    f"({int(g_dm[soft][k])}, {int(g_t[soft][k])}): width {int(g_width[soft][k])} snr {s_at[k]!r} vs {os_[soft][k]!r}")
     return r
+
+
+def level_of_width(N: np.ndarray, w0: int, levels: int) -> np.ndarray:
+    """Level of the decimated search a reported EFFECTIVE width belongs to (-1: not on the grid).  The grids of the
+    levels are disjoint: 1..w0 at level 0, then D (w0/2 + 1) .. D w0 in steps of D = 2^l."""
+    N = np.asarray(N).astype(np.int64)
+    out = np.full(N.shape, -1, dtype=np.int64)
+    out[(N >= 1) & (N <= w0)] = 0
+    for l in range(1, levels):
+        D = 1 << l
+        out[(N % D == 0) & (N // D > w0 // 2) & (N // D <= w0) & (out < 0)] = l
+    return out
+
+
+def compare_candidates_decimated(g_dm, g_t, g_snr, g_width, g_count: int, capacity: int, levels, w0: int, f_T: float,
+                                 x: np.ndarray, mu: float, sig_all: np.ndarray) -> Report:
+    """GPU list of a decimated search (unordered; record.t in the ORIGINAL series, record.width = effective width) vs the
+    brute filter of every level plane of oracle O5 (`levels` = spd_oracle.sweep_decimated).  A record belongs to the
+    level its width lies on; per level the rules are compare_candidates': equal as sets of (dm, i = t / 2^l) outside 1e-3 of
+    the threshold, SNR within tolerance, width equal outside near-ties and otherwise on the level's grid, fitting the row
+    and with an oracle SNR (re-summed over the original samples) within 1e-3 of best."""
+    r = Report()
+    g_dm = np.asarray(g_dm).astype(np.int64); g_t = np.asarray(g_t).astype(np.int64)
+    g_snr = np.asarray(g_snr, dtype=np.float64); g_width = np.asarray(g_width).astype(np.int64)
+    if g_count > capacity:
+        r.fail(f"overflow: count {g_count} > capacity {capacity} (comparison needs the whole list)")
+        return r
+    if g_dm.size != g_count:
+        r.fail(f"list length {g_dm.size} != count {g_count}")
+        return r
+    lv_of = level_of_width(g_width, w0, len(levels))
+    if np.any(lv_of < 0):
+        r.fail(f"{int(np.count_nonzero(lv_of < 0))} records whose width is on no level's grid")
+        return r
+    r.info.update(oracle_hits=0, gpu_hits=int(g_count), near_threshold_exempt=0, width_near_tie_exempt=0)
+    for L in levels:
+        lvl, D = int(L["level"]), int(L["D"])
+        o_snr, o_width, o_margin = L["snr"], L["width"], L["margin"]
+        n_dm, n_l = o_snr.shape
+        sel = lv_of == lvl
+        dm, t, sn, wd = g_dm[sel], g_t[sel], g_snr[sel], g_width[sel]
+        if np.any(t % D != 0):
+            r.fail(f"level {lvl}: record.t is not a multiple of {D}")
+            return r
+        i = t // D
+        if dm.size and (dm.min() < 0 or dm.max() >= n_dm or i.min() < 0 or i.max() >= max(n_l, 1) or n_l == 0):
+            r.fail(f"level {lvl}: candidate index out of range")
+            return r
+        gkey = dm * max(n_l, 1) + i
+        if np.unique(gkey).size != gkey.size:
+            r.fail(f"level {lvl}: duplicate (dm, t) records")
+        near = np.abs(o_snr - f_T) <= TIE
+        okey_all = np.flatnonzero((o_snr >= f_T).ravel())
+        near_flat = near.ravel()
+        okey = okey_all[~near_flat[okey_all]]
+        gk = np.sort(gkey[~near_flat[gkey]])
+        r.info["oracle_hits"] += int(okey_all.size)
+        r.info["near_threshold_exempt"] += int(near.sum())
+        if gk.size != okey.size or not np.array_equal(gk, okey):
+            missing = np.setdiff1d(okey, gk); extra = np.setdiff1d(gk, okey)
+            r.fail(f"level {lvl}: candidate sets differ: {missing.size} missing, {extra.size} extra")
+            return r
+        os_ = o_snr.ravel()[gkey]; ow = o_width.ravel()[gkey]; marg = o_margin.ravel()[gkey]
+        bad = np.abs(sn - os_) > np.maximum(SNR_ABS, SNR_REL * np.abs(os_))
+        if bad.any():
+            r.fail(f"level {lvl}: {int(bad.sum())} candidate SNRs out of tolerance")
+        mism = wd != ow
+        hard = mism & (marg > TIE)
+        if hard.any():
+            r.fail(f"level {lvl}: {int(hard.sum())} candidate widths differ outside near-ties")
+        soft = mism & ~(marg > TIE)
+        r.info["width_near_tie_exempt"] += int(soft.sum())
+        if soft.any():
+            fits = i[soft] + wd[soft] // D <= n_l
+            s_at = O.snr_at(x, mu, sig_all, dm[soft], t[soft], wd[soft].astype(np.int32))
+            worse = ~fits | ~(np.abs(s_at - os_[soft]) <= TIE)
+            if worse.any():
+                r.fail(f"level {lvl}: {int(worse.sum())} near-tie candidate widths that do not fit or are not within {TIE} of best")
+    return r
+

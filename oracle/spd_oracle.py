@@ -226,6 +226,27 @@ def sweep_decimated(x: np.ndarray, mu: float, sigma: float, sig_nmax: float, mod
     return out
 
 
+def candidates_decimated(levels, f_T: float):
+    """O4 over the levels of O5 (PAPER.md:87-93 applied to every level plane of reading A20): every level position with
+    SNR >= f_T -> one record (dm, t = i 2^l in the ORIGINAL series, snr, effective width N, level), level by level in
+    (dm, i) order.  A pulse is usually reported by several levels: nothing is merged (a plain list)."""
+    dm, t, snr, w, lv = [], [], [], [], []
+    for L in levels:
+        c_dm, c_i, c_snr, c_w = candidates(L["snr"], L["width"], f_T)
+        dm.append(c_dm); t.append(c_i * int(L["D"])); snr.append(c_snr); w.append(c_w)
+        lv.append(np.full(c_dm.size, int(L["level"]), dtype=np.int32))
+    return (np.concatenate(dm), np.concatenate(t), np.concatenate(snr), np.concatenate(w), np.concatenate(lv))
+
+
+def search_decimated(x: np.ndarray, w0: int, levels: int, mode="sqrt", f_T: float = 6.0):
+    """The decimated path O1 -> O1b -> O2 -> O5 -> O4 on one array (Nmax = w0 * 2^(levels-1)); returns a dict."""
+    m = _MODES[mode]
+    nmax = w0 * (1 << (levels - 1))
+    st = full_stats(x, nmax if m != 0 else 0)
+    lv = sweep_decimated(x, st.mean, st.sigma, st.sigma_nmax, m, w0, levels)
+    return dict(stats=st, levels=lv, cand=candidates_decimated(lv, f_T), sig=sigma_table(st.sigma, st.sigma_nmax, nmax, m))
+
+
 def search(x: np.ndarray, nmax: int, mode="sqrt", f_T: float = 6.0):
     """The whole path O1 -> O1b -> O2 -> O3 -> O4 on one array; returns a dict."""
     m = _MODES[mode]

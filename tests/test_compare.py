@@ -263,3 +263,62 @@ def test_level_plane_errors_are_rejected(dcase):
         d, i = cand[0]
         w[d, i] = 38
         assert not _lvl(dcase, 2, g_w=w)
+
+
+# ------------------------------------------------------------------------------- candidate lists of the decimated search
+def _dlist(c, thr=3.5):
+    dm, t, sn, w, lv = O.candidates_decimated(c["lv"], thr)
+    return dm, t, sn.astype(np.float32), w, lv
+
+
+def _dcmp(c, dm, t, sn, w, thr=3.5, count=None, cap=1 << 20):
+    return CMP.compare_candidates_decimated(dm, t, sn, w, len(dm) if count is None else count, cap, c["lv"], 16, thr,
+                                            c["x"], c["mu"], c["sig"])
+
+
+def test_level_of_width_partitions_the_grid():
+    N = np.arange(0, 140)
+    lv = CMP.level_of_width(N, 16, 4)
+    assert np.array_equal(np.flatnonzero(lv == 0), np.arange(1, 17))
+    assert np.array_equal(np.flatnonzero(lv == 1), np.arange(18, 33, 2))
+    assert np.array_equal(np.flatnonzero(lv == 2), np.arange(36, 65, 4))
+    assert np.array_equal(np.flatnonzero(lv == 3), np.arange(72, 129, 8))
+    assert lv[0] == -1 and lv[17] == -1 and lv[34] == -1 and lv[130] == -1
+
+
+def test_decimated_list_fp32_copy_passes_in_any_order(dcase):
+    dm, t, sn, w, lv = _dlist(dcase)
+    assert dm.size > 50 and len(set(lv.tolist())) == 4      # every level contributes
+    r = _dcmp(dcase, dm, t, sn, w)
+    assert r, str(r)
+    p = np.random.Generator(np.random.PCG64(5)).permutation(dm.size)
+    assert _dcmp(dcase, dm[p], t[p], sn[p], w[p])
+
+
+def test_decimated_list_errors_are_rejected(dcase):
+    dm, t, sn, w, lv = _dlist(dcase)
+    L2 = dcase["lv"][2]
+    k = int(np.flatnonzero((lv == 2) & (np.abs(sn - 3.5) > 0.05))[0])
+    for name, mut in [
+        ("missing", lambda a: tuple(np.delete(v, k) for v in a)),
+        ("duplicate", lambda a: tuple(np.append(v, v[k]) for v in a)),
+        ("snr", lambda a: (a[0], a[1], np.where(np.arange(a[2].size) == k, a[2] + 2e-3, a[2]).astype(np.float32), a[3])),
+        ("t not on the level's grid", lambda a: (a[0], np.where(np.arange(a[1].size) == k, a[1] + 1, a[1]), a[2], a[3])),
+        ("width off every grid", lambda a: (a[0], a[1], a[2], np.where(np.arange(a[3].size) == k, 34, a[3]))),
+    ]:
+        m = mut((dm, t, sn, w))
+        assert not _dcmp(dcase, *m), name
+    # a record moved to another level's grid by its width is an extra there and a miss here
+    w2 = w.copy(); w2[k] = 20
+    assert not _dcmp(dcase, dm, t, sn, w2)
+    # wrong width of the same level at a clear margin
+    i = t // 4
+    clear = np.flatnonzero((lv == 2) & (L2["margin"][dm, np.minimum(i, L2["snr"].shape[1] - 1)] > 0.1))
+    assert clear.size
+    w3 = w.copy(); w3[clear[0]] = 36 if w[clear[0]] != 36 else 40
+    assert not _dcmp(dcase, dm, t, sn, w3)
+    assert not _dcmp(dcase, dm, t, sn, w, count=dm.size + 1)
+    assert not _dcmp(dcase, dm, t, sn, w, cap=dm.size - 1)
+    # an extra record below the threshold
+    d, ii = np.argwhere((L2["snr"] < 3.0) & (L2["width"] > 0))[0]
+    assert not _dcmp(dcase, np.append(dm, d), np.append(t, ii * 4), np.append(sn, np.float32(L2["snr"][d, ii])), np.append(w, L2["width"][d, ii]))

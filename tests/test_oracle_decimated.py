@@ -138,3 +138,31 @@ def test_eq5_levels_use_sigma_of_the_effective_width():
     lv = O.sweep_decimated(x, 0.0, sigma, snm, "linear", W0, LEVELS)
     want = 48.0 / (math.sqrt(48) * sigma + 47 * snm / (NMAX - 1))       # eq. 5 at N = 48 with Nmax = 128
     assert lv[2]["snr"][0, 16] == pytest.approx(want, rel=1e-14) and lv[2]["width"][0, 16] == 48
+
+
+def test_candidate_list_of_the_decimated_search():
+    """O4 over the levels of O5: with one level it is the exhaustive search's list; in general it is the brute filter of
+    every level plane with t = i 2^l; an on-grid rectangular pulse heads the list at (p, W) with SNR A sqrt(W)."""
+    r = np.random.Generator(np.random.PCG64(91))
+    x = r.standard_normal((3, 4100)).astype(np.float32)
+    a = O.search_decimated(x, 16, 1, "sqrt", 3.0)
+    b = O.search(x, 16, "sqrt", 3.0)
+    for u, v in zip(a["cand"][:4], b["cand"]):
+        assert np.array_equal(u, v)
+    c = O.search_decimated(x, 16, 4, "sqrt", 3.0)
+    dm, t, snr, w, lv = c["cand"]
+    want = 0
+    got = set(zip(dm.tolist(), t.tolist(), w.tolist()))
+    assert len(got) == dm.size
+    for L in c["levels"]:
+        hit = np.argwhere(L["snr"] >= 3.0)
+        want += hit.shape[0]
+        for d, i in hit:
+            assert (int(d), int(i) * L["D"], int(L["width"][d, i])) in got
+    assert want == dm.size and np.all(snr >= 3.0)
+    A, W, p = 2.0, 48, 1024                                   # 48 = 12 * 2^2: on the grid of level 2
+    x = np.zeros((1, 4096), dtype=np.float32); x[0, p:p + W] = A
+    lv = O.sweep_decimated(x, 0.0, 1.0, float("nan"), "sqrt", 16, 4)
+    dm, t, snr, w, l = O.candidates_decimated(lv, 5.0)
+    k = int(np.argmax(snr))
+    assert (int(t[k]), int(w[k]), int(l[k])) == (p, W, 2) and snr[k] == pytest.approx(A * np.sqrt(W), rel=1e-12)
