@@ -278,12 +278,33 @@ def decimated_leg(torch, P, args, d_x, st, ws, n_dm, n_t, nmax, nmax_sigma, mode
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
+    hits_planes = int(cnt.item())
+
+    def run_fused():
+        P.spd_stats(d_x, nmax_sigma, st, ws)
+        P.spd_search_fused_decimated(d_x, st, w0, levels, mode, thr, out, cnt, ws=dws)
+    for _ in range(2):
+        run_fused()
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(steps):
+        run_fused()
+    e1.record()
+    torch.cuda.synchronize()
+    ms_fused = e0.elapsed_time(e1) / steps
+    hits_fused = int(cnt.item())
     n = n_dm * n_t
     frac_sum = sum(0.5 ** l for l in range(levels))
+    # fused: x read by the statistics and by level 0; level l >= 1 reads its series and level l < L-1 writes the next one
+    alg_fused = n * (4 + 4 + 4 * (frac_sum - 1) + 4 * sum(0.5 ** l for l in range(1, levels)))
     # bytes that must cross HBM: x read once by the statistics and once by the search, planes of every level written once and
     # their SNR read once by the candidate selection; the decimated series are intermediates (credit: none)
     alg_bytes = n * (4 + 4 + (4 + 2 + 4) * frac_sum)
-    return {"ms_per_step": ms, "w0": w0, "levels": levels, "hits": int(cnt.item()), "value": n / (ms * 1e-3), "unit": "samples/s per GPU",
+    fused = {"ms_per_step": ms_fused, "hits": hits_fused, "value": n / (ms_fused * 1e-3), "unit": "samples/s per GPU",
+             "algorithmic_bytes_per_sample": alg_fused / n, "hbm_GBps": alg_fused / (ms_fused * 1e-3) / 1e9,
+             "hbm_frac_of_measured": alg_fused / (ms_fused * 1e-3) / 1e9 / hbm_peak,
+             "note": "spd_stats + spd_search_fused_decimated: the same list with the threshold in the level kernels, no planes"}
+    return {"ms_per_step": ms, "w0": w0, "levels": levels, "hits": hits_planes, "value": n / (ms * 1e-3), "unit": "samples/s per GPU", "fused": fused,
             "algorithmic_bytes_per_sample": alg_bytes / n, "hbm_GBps": alg_bytes / (ms * 1e-3) / 1e9,
             "hbm_frac_of_measured": alg_bytes / (ms * 1e-3) / 1e9 / hbm_peak,
             "note": "spd_stats + spd_boxcar_snr_decimated + spd_candidates_decimated: widths 1..16, then 18..32 step 2, 36..64 step 4, ...; "

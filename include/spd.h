@@ -158,6 +158,17 @@ spd_status spd_candidates_decimated(const float *d_snr, const uint16_t *d_width,
                                     int levels, float threshold, spd_candidate_t *d_out, uint64_t capacity,
                                     unsigned long long *d_count, void *stream);
 
+/* The decimated search with the threshold applied in the level kernels (steps 2-4 fused, as spd_search_fused is for the
+ * exhaustive search): the level planes are never written.  Same records as spd_boxcar_snr_decimated +
+ * spd_candidates_decimated -- (dm, t, snr) bit for bit; the width of a hit is found by replaying its running sums, so it is
+ * the exact smallest arg-max among the level's widths and can differ from the plane path's only inside near-ties.
+ * Arguments, workspace and the LINEAR-mode requirement follow spd_boxcar_snr_decimated; *d_count / capacity follow
+ * spd_candidates; a LINEAR mode fed stats of another Nmax sets *d_count = UINT64_MAX, as spd_search_fused does. */
+spd_status spd_search_fused_decimated(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                                      const spd_stats_t *d_stats, int w0, int levels, spd_sigma_mode mode, float threshold,
+                                      spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,
+                                      void *d_ws, size_t ws_bytes, void *stream);
+
 /* Device bytes spd_search_host needs in d_arena for this shape and capacity. */
 size_t spd_search_host_arena_bytes(int64_t n_dm, int64_t n_t, int nmax, uint64_t capacity);
 

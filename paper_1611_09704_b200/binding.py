@@ -60,8 +60,9 @@ def lib() -> C.CDLL:
         L.spd_decimated_workspace_bytes.argtypes = [i64, i64, i32, i32]; L.spd_decimated_workspace_bytes.restype = sz
         L.spd_boxcar_snr_decimated.argtypes = [vp, i64, i64, i64, vp, i32, i32, i32, vp, vp, i64, vp, sz, vp]
         L.spd_candidates_decimated.argtypes = [vp, vp, i64, i64, i64, i32, f32, vp, u64, vp, vp]
+        L.spd_search_fused_decimated.argtypes = [vp, i64, i64, i64, vp, i32, i32, i32, f32, vp, u64, vp, vp, sz, vp]
         for f in ("spd_stats", "spd_stats_merge", "spd_boxcar_snr", "spd_candidates", "spd_search_fused", "spd_search_host",
-                  "spd_boxcar_snr_decimated", "spd_candidates_decimated", "spd_stats_rows", "spd_boxcar_snr_rows",
+                  "spd_boxcar_snr_decimated", "spd_candidates_decimated", "spd_search_fused_decimated", "spd_stats_rows", "spd_boxcar_snr_rows",
                   "spd_search_fused_rows"):
             getattr(L, f).restype = i32
         _lib = L
@@ -255,6 +256,23 @@ def spd_candidates_decimated(snr: torch.Tensor, width: torch.Tensor, n_t: int, l
         out, count = new_candidates(capacity, snr.device)
     _check(lib().spd_candidates_decimated(snr.data_ptr(), width.data_ptr(), n_dm, int(n_t), stride, int(levels), float(threshold),
                                           out.data_ptr(), out.shape[0], count.data_ptr(), _stream(stream)), "spd_candidates_decimated")
+    return out, count
+
+
+def spd_search_fused_decimated(x: torch.Tensor, stats: torch.Tensor, w0: int, levels: int, mode, threshold: float,
+                               out: Optional[torch.Tensor] = None, count: Optional[torch.Tensor] = None,
+                               capacity: int = 1 << 20, ws: Optional[torch.Tensor] = None, stream=None):
+    """Decimated search with the threshold in the level kernels (include/spd.h): one list for all levels, no planes."""
+    n_dm, n_t, rs = _plane(x, torch.float32, "x")
+    if out is None or count is None:
+        out, count = new_candidates(capacity, x.device)
+    need = int(lib().spd_decimated_workspace_bytes(n_dm, n_t, int(w0), int(levels)))
+    if need == 0:
+        raise SpdError("spd_search_fused_decimated: w0 must be 16 or 32, 1 <= levels <= 8, w0 * 2^(levels-1) <= 4096")
+    ws = torch.empty(need, dtype=torch.uint8, device=x.device) if ws is None else ws
+    _check(lib().spd_search_fused_decimated(x.data_ptr(), n_dm, n_t, rs, stats.data_ptr(), int(w0), int(levels), _MODES[mode],
+                                            float(threshold), out.data_ptr(), out.shape[0], count.data_ptr(), ws.data_ptr(),
+                                            ws.numel(), _stream(stream)), "spd_search_fused_decimated")
     return out, count
 
 

@@ -243,6 +243,43 @@ spd_status spd_candidates_decimated(const float *d_snr, const uint16_t *d_width,
     return SPD_OK;
 }
 
+spd_status spd_search_fused_decimated(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride,
+                                      const spd_stats_t *d_stats, int w0, int levels, spd_sigma_mode mode, float threshold,
+                                      spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,
+                                      void *d_ws, size_t ws_bytes, void *stream)
+{
+    if (!d_x || !d_stats || !d_count || (!d_out && capacity > 0) || !d_ws || !shape_ok(n_dm, n_t, row_stride) || !dec_ok(w0, levels, n_t))
+        return SPD_ERR_INVALID_ARG;
+    if ((int)mode < 0 || (int)mode > 2 || threshold != threshold || (reinterpret_cast<uintptr_t>(d_ws) & 255) != 0) return SPD_ERR_INVALID_ARG;
+    if (ws_bytes < spd_decimated_workspace_bytes(n_dm, n_t, w0, levels)) return SPD_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    unsigned char *p = reinterpret_cast<unsigned char *>(d_ws);
+    float *table = reinterpret_cast<float *>(p);                  p += align_up(spd_workspace_bytes(n_dm, n_t, w0), 256);
+    spd_stats_t *lst = reinterpret_cast<spd_stats_t *>(p);        p += 256;
+    float *buf[2] = {nullptr, nullptr};
+    if (levels > 1) { buf[0] = reinterpret_cast<float *>(p); p += align_up((size_t)n_dm * (size_t)dec_stride(dec_n(n_t, 1)) * 4, 256); }
+    if (levels > 2) { buf[1] = reinterpret_cast<float *>(p); }
+    const int nmax_total = w0 << (levels - 1);
+    const bool rc = sweep_uses_constant_table(w0, (int)mode);
+    if (cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s) != cudaSuccess) return SPD_ERR_CUDA;
+    const float *src = d_x;
+    int64_t src_stride = row_stride;
+    for (int l = 0; l < levels; ++l) {
+        const int D = 1 << l;
+        const int64_t n_l = dec_n(n_t, l);
+        if (n_l < 1) break;
+        float *nxt = nullptr;                                     // the search of level l also writes x_{l+1}; the two buffers alternate
+        int64_t nxt_stride = 0;
+        if (l + 1 < levels && dec_n(n_t, l + 1) >= 1) { nxt = buf[l & 1]; nxt_stride = dec_stride(dec_n(n_t, l + 1)); }
+        if (launch_level_stats(d_stats, D, lst, s) != cudaSuccess) return SPD_ERR_CUDA;
+        if (!rc && launch_sigma_table(d_stats, w0, (int)mode, table, s, D, nmax_total) != cudaSuccess) return SPD_ERR_CUDA;
+        if (launch_search_level(src, n_dm, n_l, src_stride, lst, table, w0, l == 0 ? 0 : w0 / 2, D, rc, threshold, d_out, capacity,
+                                d_count, nxt, nxt_stride, s) != cudaSuccess) return SPD_ERR_CUDA;
+        src = nxt; src_stride = nxt_stride;
+    }
+    return SPD_OK;
+}
+
 // arena layout of spd_search_host: x | candidates | stats | count | workspace
 size_t spd_search_host_arena_bytes(int64_t n_dm, int64_t n_t, int nmax, uint64_t capacity)
 {

@@ -51,6 +51,9 @@ cudaError_t launch_level_stats(const spd_stats_t *st, int D, spd_stats_t *out, c
 cudaError_t launch_sweep_level(const float *xl, int64_t n_dm, int64_t n_l, int64_t xl_stride, const spd_stats_t *d_stats_level,
                                const float *d_table, int w0, int wmin, int wscale, bool rc, float *snr, uint16_t *width,
                                int64_t out_stride, float *dec_out, int64_t dec_stride, cudaStream_t s);
+cudaError_t launch_search_level(const float *xl, int64_t n_dm, int64_t n_l, int64_t xl_stride, const spd_stats_t *d_stats_level,
+                                const float *d_table, int w0, int wmin, int wscale, bool rc, float threshold, spd_candidate_t *out,
+                                unsigned long long capacity, unsigned long long *d_count, float *dec_out, int64_t dec_stride, cudaStream_t s);
 bool sweep_uses_constant_table(int nmax, int mode);      // eq. 4 with nmax a multiple of 8: r_w = 1/sqrt(w) from the constant bank, no table launch
 cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, const spd_stats_t *d_stats,
                          const float *d_table, int nmax, bool rc, float *snr, uint16_t *width,

@@ -722,6 +722,134 @@ boxcar_search_fused(const float *__restrict__ x, int64_t n_t, int64_t row_stride
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// One level of the FUSED decimated search (spd_search_fused_decimated; PAPER.md:97 + :87-93, reading A20): the width loop
+// of boxcar_search_fused on the decimated series x_l for the level's widths w' = wmin + 1 .. nmax (nmax = w0 <= 32; the
+// widths up to wmin, a multiple of 8, are only summed: they belong to the finer levels), threshold in the kernel, no
+// planes.  A hit becomes the record (row, t = i wscale, snr, width = w' wscale), wscale = 2^l.  Like the narrow plane
+// kernel of a level it also writes the next level's series, x_{l+1}[i] = x_l[2i] + x_l[2i+1], from the tile it has staged.
+__device__ __forceinline__ void sum8(float2 (&B)[SW_R], float2 (&W)[SW_R], const float2 *__restrict__ zp)
+{
+#pragma unroll
+    for (int u = 0; u < 8; u += 2) {
+        const float4 nq = *reinterpret_cast<const float4 *>(zp + u);
+        const float2 n0 = make_float2(nq.x, nq.y), n1 = make_float2(nq.z, nq.w);
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) {
+            B[j] = __fadd2_rn(B[j], W[(j + u) & 7]);
+            B[j] = __fadd2_rn(B[j], (j == SW_R - 1) ? n0 : W[(j + u + 1) & 7]);
+        }
+        W[u] = n0;
+        W[u + 1] = n1;
+    }
+}
+
+__device__ __noinline__ int replay_width_level(const float *__restrict__ zh, int pos, const float *__restrict__ rtf, int nmax, int wmin, float best)
+{
+    float b = 0.f;
+    for (int w = 1; w <= nmax; ++w) {
+        b = __fadd_rn(b, zh[2 * zpad(pos + w - 1)]);
+        if (w > wmin && __fmul_rn(b, rtf[w - 1]) == best) return w;
+    }
+    return nmax;                                   // not reached for finite input
+}
+
+template <int SW_THREADS, bool RC>
+__global__ void __launch_bounds__(SW_THREADS, 512 / SW_THREADS)
+boxcar_search_fused_level(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
+                          const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax, int wmin, int wscale,
+                          float threshold, spd_candidate_t *__restrict__ cand, unsigned long long capacity,
+                          unsigned long long *__restrict__ count, float *__restrict__ dec_out, int64_t dec_stride)
+{
+    constexpr int SW_SUB = SW_THREADS * SW_R, SW_TILE = 2 * SW_SUB;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const FusedSmem lay(nmax, SW_THREADS);
+    float2 *Z   = reinterpret_cast<float2 *>(smem_raw + lay.z);
+    float  *raw = reinterpret_cast<float *>(smem_raw + lay.raw);
+    float  *rtf = reinterpret_cast<float *>(smem_raw + lay.rtf);
+
+    const int tid = threadIdx.x;
+    const int nblk = sw_nblk(nmax);
+    const int H = sw_halo(nmax);
+    const int LRAW = SW_TILE + H, LZ = SW_SUB + H;
+    const Norm norm(st);
+    const float NINF = __int_as_float(0xff800000);
+
+    for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = RC ? c_isqrt.v[w] : __ldg(table + w);
+    // a NaN reciprocal table (LINEAR mode fed stats of another Nmax) is reported as count = ~0 (spd.h), as in boxcar_search_fused
+    if (!RC && blockIdx.x == 0 && tid == 0) { const float r0 = __ldg(table); if (r0 != r0) *count = ~0ULL; }
+
+    int64_t tile = blockIdx.x;
+    TilePos pos(blockIdx.x, tiles_per_row);
+    __shared__ unsigned long long stage_bar;
+    TileStager stg;
+    stg.init(&stage_bar, tid);
+    if (tile < total_tiles) stg.stage<SW_THREADS, true>(raw, x, n_t, row_stride, pos, LRAW, tid);
+
+    for (; tile < total_tiles; tile += gridDim.x) {
+        const int64_t row = pos.row;
+        const int64_t T0 = (int64_t)pos.tr * SW_TILE;
+        pos = pos.next(gridDim.x, tiles_per_row);                                  // the tile after this one
+        stg.wait();
+        __syncthreads();                           // raw tile landed; everyone is done with the previous Z
+
+        float2 B[SW_R], W[SW_R], best[SW_R];
+        if (dec_out == nullptr) load_norm_group<SW_SUB, RC>(raw, tid, norm, W);
+        else {                                     // the thread's own samples, summed in pairs: the next level's series
+            float4 sa, sb;
+            load_norm_group<SW_SUB, RC, true>(raw, tid, norm, W, &sa, &sb);
+            const int64_t n_next = n_t >> 1;
+            const int64_t ia = (T0 + SW_R * tid) >> 1, ib = ia + SW_SUB / 2;
+            float *da = dec_out + row * dec_stride + ia, *db = dec_out + row * dec_stride + ib;
+            const bool al = ((reinterpret_cast<uintptr_t>(dec_out + row * dec_stride) & 15) == 0);
+            if (al && ia + 3 < n_next) *reinterpret_cast<float4 *>(da) = sa;
+            else { const float t[4] = {sa.x, sa.y, sa.z, sa.w}; for (int k = 0; k < 4; ++k) if (ia + k < n_next) da[k] = t[k]; }
+            if (al && ib + 3 < n_next) *reinterpret_cast<float4 *>(db) = sb;
+            else { const float t[4] = {sb.x, sb.y, sb.z, sb.w}; for (int k = 0; k < 4; ++k) if (ib + k < n_next) db[k] = t[k]; }
+        }
+        store_group(Z, tid, W);
+        for (int g = SW_THREADS + tid; 8 * g < LZ; g += SW_THREADS) {      // the halo positions past the sub-tile
+            float2 v[SW_R];
+            load_norm_group<SW_SUB, RC>(raw, g, norm, v);
+            store_group(Z, g, v);
+        }
+        __syncthreads();                           // Z complete; raw is free again
+        if (tile + gridDim.x < total_tiles) stg.stage<SW_THREADS, true>(raw, x, n_t, row_stride, pos, LRAW, tid);
+
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); }
+        {
+            const float2 *zp = Z + 10 * (tid + 1);
+            const float *rp = rtf;
+            for (int kb = 0; kb < nblk; ++kb, zp += 10, rp += 8) {
+                if (8 * (kb + 1) <= wmin) sum8(B, W, zp);
+                else sweep8<RC>(B, W, best, best, zp, rp, 8 * kb);
+            }
+        }
+
+        // ---- threshold; hits replay their own running sums to get the width ------------------------------------------
+        const int64_t ta = T0 + SW_R * tid, tb = ta + SW_SUB;
+        bool any = false;
+#pragma unroll
+        for (int j = 0; j < SW_R; ++j) any |= (best[j].x >= threshold && ta + j < n_t) || (best[j].y >= threshold && tb + j < n_t);
+        if (__any_sync(0xffffffffu, any)) {
+            const float *zf = reinterpret_cast<const float *>(Z);
+#pragma unroll
+            for (int j = 0; j < SW_R; ++j) {
+                const bool ha = best[j].x >= threshold && ta + j < n_t;
+                const bool hb = best[j].y >= threshold && tb + j < n_t;
+                int wa = 1, wb = 1;
+                if (ha) wa = replay_width_level(zf, SW_R * tid + j, rtf, nmax, wmin, best[j].x);
+                if (hb) wb = replay_width_level(zf + 1, SW_R * tid + j, rtf, nmax, wmin, best[j].y);
+                __syncwarp();
+                append_candidate(ha, (uint32_t)row, (uint32_t)((ta + j) * wscale), best[j].x, (uint32_t)(wa * wscale), cand, capacity, count);
+                append_candidate(hb, (uint32_t)row, (uint32_t)((tb + j) * wscale), best[j].y, (uint32_t)(wb * wscale), cand, capacity, count);
+            }
+        }
+    }
+    cp_async_commit_wait_all();
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // Narrow searches (nmax <= SW_NARROW_NMAX = 32, the room of a 5-bit tag): the fixed per-sample cost of the general
 // kernel (prefix scan + width search) is larger than the width loop itself, so here the arg-max rides along with the
 // maximum: beside the exact running maximum a second one is kept over TAGGED values, (bits(s) & ~31) | (32 - w), one
@@ -1008,6 +1136,30 @@ cudaError_t launch_sweep_level(const float *xl, int64_t n_dm, int64_t n_l, int64
     } else {
         if ((e = persistent_grid(boxcar_snr_sweep_narrow<NT, false, true>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
         boxcar_snr_sweep_narrow<NT, false, true><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, snr, width, wmin, wscale, out_stride, 0, dec_out, dec_stride);
+    }
+    return cudaGetLastError();
+}
+
+// one level of the fused decimated search (w0 <= 32): threshold in the kernel, hits appended to one list for all levels
+cudaError_t launch_search_level(const float *xl, int64_t n_dm, int64_t n_l, int64_t xl_stride, const spd_stats_t *d_stats_level,
+                                const float *d_table, int w0, int wmin, int wscale, bool rc, float threshold, spd_candidate_t *out,
+                                unsigned long long capacity, unsigned long long *d_count, float *dec_out, int64_t dec_stride, cudaStream_t s)
+{
+    constexpr int NT = 64, TILE = 2 * NT * SW_R;
+    if (n_l <= 0) return cudaSuccess;
+    const int tpr = (int)((n_l + TILE - 1) / TILE);
+    const int64_t tiles = n_dm * (int64_t)tpr;
+    const FusedSmem lay(w0, NT);
+    unsigned grid = 0;
+    cudaError_t e;
+    if (rc) {
+        if ((e = persistent_grid(boxcar_search_fused_level<NT, true>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_search_fused_level<NT, true><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, wmin, wscale,
+                                                                        threshold, out, capacity, d_count, dec_out, dec_stride);
+    } else {
+        if ((e = persistent_grid(boxcar_search_fused_level<NT, false>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+        boxcar_search_fused_level<NT, false><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, wmin, wscale,
+                                                                         threshold, out, capacity, d_count, dec_out, dec_stride);
     }
     return cudaGetLastError();
 }

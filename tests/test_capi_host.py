@@ -86,7 +86,8 @@ def test_product_path_has_no_cpu_fallback():
 
 
 def test_round2_entry_points_validate_arguments(L):
-    """spd_stats_rows / spd_boxcar_snr_rows / spd_search_fused_rows / spd_boxcar_snr_decimated / spd_candidates_decimated."""
+    """spd_stats_rows / spd_boxcar_snr_rows / spd_search_fused_rows / spd_boxcar_snr_decimated / spd_candidates_decimated /
+    spd_search_fused_decimated."""
     fake = C.c_void_p(4096)
     INV, WS = 1, 3
     L.spd_decimated_level_offset.restype = C.c_int64
@@ -102,6 +103,9 @@ def test_round2_entry_points_validate_arguments(L):
     assert L.spd_boxcar_snr_decimated(fake, *a, fake, 16, 2, 0, fake, fake, C.c_int64(100), fake, C.c_size_t(1 << 30), None) == INV   # plane_stride too short
     assert L.spd_boxcar_snr_decimated(fake, *a, fake, 16, 2, 0, fake, fake, C.c_int64(8192), fake, C.c_size_t(64), None) == WS
     assert L.spd_candidates_decimated(fake, fake, C.c_int64(2), C.c_int64(4096), C.c_int64(100), 2, C.c_float(5.0), fake, C.c_uint64(10), fake, None) == INV
+    assert L.spd_search_fused_decimated(fake, *a, fake, 8, 2, 0, C.c_float(5.0), fake, C.c_uint64(4), fake, fake, C.c_size_t(1 << 30), None) == INV
+    assert L.spd_search_fused_decimated(fake, *a, fake, 16, 2, 0, C.c_float(float("nan")), fake, C.c_uint64(4), fake, fake, C.c_size_t(1 << 30), None) == INV
+    assert L.spd_search_fused_decimated(fake, *a, fake, 16, 2, 0, C.c_float(5.0), fake, C.c_uint64(4), fake, fake, C.c_size_t(64), None) == WS
     L.spd_workspace_bytes_rows.restype = C.c_size_t
     assert L.spd_workspace_bytes_rows(C.c_int64(100), C.c_int64(4096), 64) >= 100 * 80 * 4
     assert L.spd_stats_rows(fake, C.c_int64(0), C.c_int64(10), C.c_int64(10), 0, fake, fake, C.c_size_t(1 << 20), None) == INV

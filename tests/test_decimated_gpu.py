@@ -129,3 +129,76 @@ def test_decimated_argument_errors(P):
     for w0, levels in [(8, 2), (16, 0), (16, 9), (32, 8 + 1), (24, 2)]:
         with pytest.raises(P.SpdError):
             P.spd_boxcar_snr_decimated(x, st, w0, levels)
+
+
+# ---------------------------------------------------------------------------- fused decimated search (no planes)
+def _run_fused(P, x, w0, levels, mode="sqrt", stats=None, thr=5.0, stride=None):
+    """spd_search_fused_decimated against the candidate list of oracle O5 + O4 (level by level: set of (dm, t) outside 1e-3
+    of the threshold, SNR tolerance, width / near-tie rules), and against the plane path's list (same (dm, t, snr) bits)."""
+    from gpu_util import to_dev
+    nmax = w0 << (levels - 1)
+    o = O.full_stats(x, nmax if mode != "sqrt" else 0) if stats is None else stats
+    st = P.write_stats(o.mean, o.sigma, o.sigma_nmax, o.nmax_of_sigma)
+    d = to_dev(x, stride)
+    out, cnt = P.spd_search_fused_decimated(d, st, w0, levels, mode, thr, capacity=1 << 20)
+    rec, total = P.read_candidates(out, cnt)
+    lv = O.sweep_decimated(x, o.mean, o.sigma, o.sigma_nmax, mode, w0, levels)
+    sig_all = O.sigma_table(o.sigma, o.sigma_nmax, nmax, mode)
+    r = CMP.compare_candidates_decimated(rec["dm"], rec["t"], rec["snr"], rec["width"], total, 1 << 20, lv, w0, thr, x, o.mean, sig_all)
+    assert r, str(r)
+    snr, width = P.spd_boxcar_snr_decimated(d, st, w0, levels, mode)
+    out2, cnt2 = P.spd_candidates_decimated(snr, width, x.shape[1], levels, thr, capacity=1 << 20)
+    rec2, total2 = P.read_candidates(out2, cnt2)
+    assert total == total2
+    lvl = CMP.level_of_width(rec["width"], w0, levels)
+    lvl2 = CMP.level_of_width(rec2["width"], w0, levels)
+    a = np.lexsort((rec["t"], rec["dm"], lvl)); b = np.lexsort((rec2["t"], rec2["dm"], lvl2))
+    for k in ("dm", "t", "snr"):
+        assert rec[k][a].tobytes() == rec2[k][b].tobytes(), k
+    assert (rec["width"][a] != rec2["width"][b]).mean() <= 0.02
+    return rec, r.info
+
+
+@pytest.mark.parametrize("n_dm,n_t,w0,levels", [(2, 4096, 16, 1), (2, 4096, 16, 4), (3, 5003, 16, 4), (1, 2049, 32, 3),
+                                                (2, 1000, 16, 6), (1, 40, 16, 2), (2, 9001, 32, 8)])
+def test_fused_decimated_integer_data(P, n_dm, n_t, w0, levels):
+    x = rng(700 + n_t).integers(-4, 6, size=(n_dm, n_t)).astype(np.float32)
+    rec, info = _run_fused(P, x, w0, levels, "sqrt", O.Stats(0, 0.0, 0.0, 0.0, 1.0), thr=4.0)
+    assert info["gpu_hits"] > 0
+
+
+@pytest.mark.parametrize("mode", ["sqrt", "linear", "anchored"])
+@pytest.mark.parametrize("mu,sigma", [(0.0, 1.0), (100.0, 20.0)])
+def test_fused_decimated_noise_all_modes(P, mode, mu, sigma):
+    x = (mu + sigma * rng(800).standard_normal((3, 7001))).astype(np.float32)
+    x[1, 2000:2090] += 0.8 * sigma
+    rec, info = _run_fused(P, x, 16, 4, mode, thr=3.5, stride=7008 if mode == "linear" else None)
+    assert info["gpu_hits"] > (30 if mode == "sqrt" else 3)       # eq. 5 flattens the SNR: fewer samples above the threshold
+
+
+def test_fused_decimated_on_grid_pulse_and_overflow(P):
+    n_t, A, W, p = 8192, 2.0, 48, 3200                      # 48 = 12 * 2^2
+    x = np.zeros((1, n_t), dtype=np.float32); x[0, p:p + W] = A
+    d = torch.from_numpy(x).cuda()
+    out, cnt = P.spd_search_fused_decimated(d, P.write_stats(0.0, 1.0), 16, 4, "sqrt", 5.0, capacity=1 << 16)
+    rec, total = P.read_candidates(out, cnt)
+    k = int(np.argmax(rec["snr"]))
+    assert (int(rec["t"][k]), int(rec["width"][k])) == (p, W) and float(rec["snr"][k]) == pytest.approx(A * math.sqrt(W), rel=3e-7)
+    out, cnt = P.spd_search_fused_decimated(d, P.write_stats(0.0, 1.0), 16, 4, "sqrt", 5.0, capacity=8)   # overflow convention
+    assert int(cnt.item()) == total > 8
+
+
+def test_fused_decimated_linear_with_wrong_nmax_reports_misuse(P):
+    x = torch.randn((2, 4096), device="cuda")
+    st = P.spd_stats(x, 64)                                  # sigma_Nmax measured for 64, the search wants 128
+    out, cnt = P.spd_search_fused_decimated(x, st, 16, 4, "linear", 5.0)
+    with pytest.raises(P.SpdError):
+        P.read_candidates(out, cnt)
+
+
+def test_fused_decimated_config3_rows(P):
+    cfg = gen.get_config(3)
+    rows = sorted(set(gen.pulse_rows(cfg)[:12]) | set(range(0, 24)))
+    x = gen.make_rows(cfg, rows)
+    rec, info = _run_fused(P, x, 16, 4, "sqrt", O.stats(x), thr=cfg.threshold)
+    assert info["gpu_hits"] > 0
