@@ -753,7 +753,7 @@ __device__ __noinline__ int replay_width_level(const float *__restrict__ zh, int
     return nmax;                                   // not reached for finite input
 }
 
-template <int SW_THREADS, bool RC>
+template <int SW_THREADS, bool RC, int W0, bool LEVEL0>
 __global__ void __launch_bounds__(SW_THREADS, 512 / SW_THREADS)
 boxcar_search_fused_level(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                           const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax, int wmin, int wscale,
@@ -818,11 +818,13 @@ boxcar_search_fused_level(const float *__restrict__ x, int64_t n_t, int64_t row_
 #pragma unroll
         for (int j = 0; j < SW_R; ++j) { B[j] = make_float2(0.f, 0.f); best[j] = make_float2(NINF, NINF); }
         {
+            // W0 and the level kind are compile-time: straight-line blocks, r_w of eq. 4 at constant offsets of the constant bank
             const float2 *zp = Z + 10 * (tid + 1);
-            const float *rp = rtf;
-            for (int kb = 0; kb < nblk; ++kb, zp += 10, rp += 8) {
-                if (8 * (kb + 1) <= wmin) sum8(B, W, zp);
-                else sweep8<RC>(B, W, best, best, zp, rp, 8 * kb);
+            constexpr int NB = W0 / 8, FIRST = LEVEL0 ? 0 : NB / 2;      // blocks below FIRST are only summed (wmin = W0 / 2)
+#pragma unroll
+            for (int kb = 0; kb < NB; ++kb) {
+                if (kb < FIRST) sum8(B, W, zp + 10 * kb);
+                else sweep8<RC>(B, W, best, best, zp + 10 * kb, rtf + 8 * kb, 8 * kb);
             }
         }
 
@@ -1140,28 +1142,40 @@ cudaError_t launch_sweep_level(const float *xl, int64_t n_dm, int64_t n_l, int64
     return cudaGetLastError();
 }
 
-// one level of the fused decimated search (w0 <= 32): threshold in the kernel, hits appended to one list for all levels
+template <bool RC, int W0, bool LEVEL0>
+static cudaError_t launch_search_level_t(const float *xl, int64_t n_dm, int64_t n_l, int64_t xl_stride, const spd_stats_t *d_stats_level,
+                                         const float *d_table, int wscale, float threshold, spd_candidate_t *out,
+                                         unsigned long long capacity, unsigned long long *d_count, float *dec_out, int64_t dec_stride, cudaStream_t s)
+{
+    constexpr int NT = 64, TILE = 2 * NT * SW_R;
+    const int tpr = (int)((n_l + TILE - 1) / TILE);
+    const int64_t tiles = n_dm * (int64_t)tpr;
+    const FusedSmem lay(W0, NT);
+    unsigned grid = 0;
+    cudaError_t e;
+    if ((e = persistent_grid(boxcar_search_fused_level<NT, RC, W0, LEVEL0>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
+    boxcar_search_fused_level<NT, RC, W0, LEVEL0><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, W0,
+                                                                              LEVEL0 ? 0 : W0 / 2, wscale, threshold, out, capacity, d_count,
+                                                                              dec_out, dec_stride);
+    return cudaGetLastError();
+}
+
+// one level of the fused decimated search (w0 = 16 or 32; wmin = 0 at level 0, w0 / 2 above): threshold in the kernel, hits
+// appended to one list for all levels
 cudaError_t launch_search_level(const float *xl, int64_t n_dm, int64_t n_l, int64_t xl_stride, const spd_stats_t *d_stats_level,
                                 const float *d_table, int w0, int wmin, int wscale, bool rc, float threshold, spd_candidate_t *out,
                                 unsigned long long capacity, unsigned long long *d_count, float *dec_out, int64_t dec_stride, cudaStream_t s)
 {
-    constexpr int NT = 64, TILE = 2 * NT * SW_R;
     if (n_l <= 0) return cudaSuccess;
-    const int tpr = (int)((n_l + TILE - 1) / TILE);
-    const int64_t tiles = n_dm * (int64_t)tpr;
-    const FusedSmem lay(w0, NT);
-    unsigned grid = 0;
-    cudaError_t e;
-    if (rc) {
-        if ((e = persistent_grid(boxcar_search_fused_level<NT, true>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_search_fused_level<NT, true><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, wmin, wscale,
-                                                                        threshold, out, capacity, d_count, dec_out, dec_stride);
-    } else {
-        if ((e = persistent_grid(boxcar_search_fused_level<NT, false>, NT, lay.total, tiles, &grid)) != cudaSuccess) return e;
-        boxcar_search_fused_level<NT, false><<<grid, NT, lay.total, s>>>(xl, n_l, xl_stride, tpr, tiles, d_stats_level, d_table, w0, wmin, wscale,
-                                                                         threshold, out, capacity, d_count, dec_out, dec_stride);
+    if ((w0 != 16 && w0 != 32) || (wmin != 0 && wmin != w0 / 2)) return cudaErrorInvalidValue;
+#define SPD_LEVEL(RC_, W0_, L0_) launch_search_level_t<RC_, W0_, L0_>(xl, n_dm, n_l, xl_stride, d_stats_level, d_table, wscale, threshold, out, capacity, d_count, dec_out, dec_stride, s)
+    if (w0 == 16) {
+        if (wmin == 0) return rc ? SPD_LEVEL(true, 16, true) : SPD_LEVEL(false, 16, true);
+        return rc ? SPD_LEVEL(true, 16, false) : SPD_LEVEL(false, 16, false);
     }
-    return cudaGetLastError();
+    if (wmin == 0) return rc ? SPD_LEVEL(true, 32, true) : SPD_LEVEL(false, 32, true);
+    return rc ? SPD_LEVEL(true, 32, false) : SPD_LEVEL(false, 32, false);
+#undef SPD_LEVEL
 }
 
 }  // namespace spd
