@@ -26,20 +26,23 @@ constexpr int REPS = 4;
 
 __device__ __forceinline__ float fmax3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }
 
-enum Mode { FADD, FMUL, FFMA, FMNMX, FMNMX3, FADD2, FMUL2, FMUL2_BCAST, FFMA2, MIX_SCALAR, MIX_SCALAR_RCONST, MIX_PACKED, MIX_PACKED_RCONST, MIX_PACKED_RCONST_ARGMAX, NMODES };
+enum Mode { FADD, FMUL, FFMA, FMNMX, FMNMX3, FADD2, FMUL2, FMUL2_BCAST, FFMA2, MIX_SCALAR, MIX_SCALAR_RCONST, MIX_PACKED, MIX_PACKED_RCONST, MIX_PACKED_RCONST_ARGMAX, LOP3_OP, IADD3_OP, MIX_NARROW, MIX_NARROW_TAGONLY, NMODES };
 static const char *mode_name[NMODES] = {
     "FADD  r,r", "FMUL  r,r", "FFMA  r,r,r", "FMNMX r,r x2 (ptxas fuses two into one FMNMX3)", "FMNMX3 r,r,r", "FADD2 rr,rr", "FMUL2 rr,rr", "FMUL2 rr,r (scalar broadcast)",
     "FFMA2 rr,rr,rr", "loop mix, scalar: 2 FADD + 2 FMUL + 1 FMNMX3 per 2 pairs", "loop mix, scalar, r_w from the constant bank",
     "loop mix, packed: 2 FADD2 + 2 FMUL2(bcast) + 2 FMNMX3 per 4 pairs", "loop mix, packed, r_w from the constant bank (uniform register)",
-    "loop mix, packed, r_w constant, + block arg-max (ping-pong maxima, FSETP + SEL per sum per 8 widths)"};
+    "loop mix, packed, r_w constant, + block arg-max (ping-pong maxima, FSETP + SEL per sum per 8 widths)",
+    "LOP3 r,r,r", "IADD3 r,r",
+    "narrow mix (sweep8_tagged): loop mix + per pair one LOP3 tag and half an FMNMX3 over the tagged values",
+    "narrow mix without the exact maximum (tagged maximum only; not used: the SNR would lose its 5 low bits)"};
 // warp instructions per repetition, and (sample, width) pairs per repetition per lane (0 = not a loop mix)
-static const int mode_instr[NMODES] = {16, 16, 16, 8, 16, 8, 8, 8, 8, 40, 40, 48, 48, 112};
-static const int mode_pairs[NMODES] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 16, 16, 32, 32, 64};
+static const int mode_instr[NMODES] = {16, 16, 16, 8, 16, 8, 8, 8, 8, 40, 40, 48, 48, 112, 16, 16, 96, 80};
+static const int mode_pairs[NMODES] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 16, 16, 32, 32, 64, 0, 0, 32, 32};
 
 struct RTable { float r[8]; };
 
 template <int MODE>
-__global__ void __launch_bounds__(128) bench_kernel(float *out, long long *clk, int iters, float fa, float fb, RTable rt)
+__global__ void __launch_bounds__(128) bench_kernel(float *out, long long *clk, int iters, float fa, float fb, RTable rt, int tagmask)
 {
     extern __shared__ float dummy[];
     float a[NA], w[NA], m[NA];
@@ -95,6 +98,31 @@ __global__ void __launch_bounds__(128) bench_kernel(float *out, long long *clk, 
                     a[j] = __fadd_rn(a[j], w[(j + 2 * rep + 1) & 15]);
                     const float s1 = __fmul_rn(a[j], q1);
                     m[j] = fmax3(m[j], s0, s1);
+                }
+            } else if (MODE == LOP3_OP) {
+#pragma unroll
+                for (int j = 0; j < NA; ++j) { int d; asm volatile("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(d) : "r"(__float_as_int(a[j])), "r"(__float_as_int(w[j])), "r"(__float_as_int(m[j]))); a[j] = __int_as_float(d); }
+            } else if (MODE == IADD3_OP) {
+#pragma unroll
+                for (int j = 0; j < NA; ++j) { int d; asm volatile("add.s32 %0, %1, %2;" : "=r"(d) : "r"(__float_as_int(a[j])), "r"(__float_as_int(w[j]))); a[j] = __int_as_float(d); }
+            } else if (MODE == MIX_NARROW || MODE == MIX_NARROW_TAGONLY) {
+                // the width loop of boxcar_snr_sweep_narrow: the loop mix plus a second maximum over values whose 5 low mantissa
+                // bits carry the width (one LOP3 per value); O2 plays the tagged maxima
+                const float2 q0 = make_float2(rt.r[2 * rep], rt.r[2 * rep]), q1 = make_float2(rt.r[2 * rep + 1], rt.r[2 * rep + 1]);
+                const int c0 = 31 - 2 * rep, c1 = c0 - 1;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    A2[j] = __fadd2_rn(A2[j], W2[(j + 2 * rep) & 7]);
+                    const float2 s0 = __fmul2_rn(A2[j], q0);
+                    A2[j] = __fadd2_rn(A2[j], W2[(j + 2 * rep + 1) & 7]);
+                    const float2 s1 = __fmul2_rn(A2[j], q1);
+                    if (MODE == MIX_NARROW) { M2[j].x = fmax3(M2[j].x, s0.x, s1.x); M2[j].y = fmax3(M2[j].y, s0.y, s1.y); }
+                    float t0, t1, t2, t3;
+                    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=f"(t0) : "f"(s0.x), "r"(tagmask), "r"(c0));
+                    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=f"(t1) : "f"(s1.x), "r"(tagmask), "r"(c1));
+                    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=f"(t2) : "f"(s0.y), "r"(tagmask), "r"(c0));
+                    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=f"(t3) : "f"(s1.y), "r"(tagmask), "r"(c1));
+                    O2[j].x = fmax3(O2[j].x, t0, t1); O2[j].y = fmax3(O2[j].y, t2, t3);
                 }
             } else if (MODE == MIX_PACKED || MODE == MIX_PACKED_RCONST) {
                 // the same for 8 packed running sums (two samples each): what sweep8 in sweep.cu issues
@@ -167,7 +195,7 @@ static void run_mode(int k, float *d_out, long long *d_clk, int sms, int smem_pe
     float best_ms = 1e30f; long long clk[2] = {0, 0};
     for (int t = 0; t < 4; ++t) {                                  // first run is the warm-up; best of the next three
         CK(cudaEventRecord(e0));
-        bench_kernel<MODE><<<sms * k, 128, smem>>>(d_out, d_clk, iters, 1.0f, 1.000001f, rt);
+        bench_kernel<MODE><<<sms * k, 128, smem>>>(d_out, d_clk, iters, 1.0f, 1.000001f, rt, ~31);
         CK(cudaEventRecord(e1));
         CK(cudaEventSynchronize(e1));
         float ms; CK(cudaEventElapsedTime(&ms, e0, e1));
@@ -212,5 +240,9 @@ int main()
     run_all<MIX_PACKED>(d_out, d_clk, sms, smem_per_sm);
     run_all<MIX_PACKED_RCONST>(d_out, d_clk, sms, smem_per_sm);
     run_all<MIX_PACKED_RCONST_ARGMAX>(d_out, d_clk, sms, smem_per_sm);
+    run_all<LOP3_OP>(d_out, d_clk, sms, smem_per_sm);
+    run_all<IADD3_OP>(d_out, d_clk, sms, smem_per_sm);
+    run_all<MIX_NARROW>(d_out, d_clk, sms, smem_per_sm);
+    run_all<MIX_NARROW_TAGONLY>(d_out, d_clk, sms, smem_per_sm);
     return 0;
 }
