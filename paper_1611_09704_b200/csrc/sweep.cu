@@ -754,7 +754,7 @@ __device__ __noinline__ int replay_width_level(const float *__restrict__ zh, int
 }
 
 template <int SW_THREADS, bool RC, int W0, bool LEVEL0>
-__global__ void __launch_bounds__(SW_THREADS, 512 / SW_THREADS)
+__global__ void __launch_bounds__(SW_THREADS, 640 / SW_THREADS)
 boxcar_search_fused_level(const float *__restrict__ x, int64_t n_t, int64_t row_stride, int tiles_per_row, int64_t total_tiles,
                           const spd_stats_t *__restrict__ st, const float *__restrict__ table, int nmax, int wmin, int wscale,
                           float threshold, spd_candidate_t *__restrict__ cand, unsigned long long capacity,
