@@ -3,8 +3,9 @@
 //
 //   B_N(t) = sum_{k<N} x[t+k];  SNR_N(t) = (B_N(t) - N mu) / sigma_N;  snr[t] = max_N, width[t] = smallest arg-max.
 //
-// Three kernels share one width loop (sweep8): boxcar_snr_sweep (planes, any nmax), boxcar_snr_sweep_narrow (planes,
-// nmax <= 32) and boxcar_search_fused (threshold in the kernel, no planes).
+// Four kernels share one width loop (sweep8 / sweep8_tagged): boxcar_snr_sweep (planes, any nmax), boxcar_snr_sweep_narrow
+// (planes, nmax <= 32; also one level of the decimated search), boxcar_search_fused (threshold in the kernel, no planes) and
+// boxcar_search_fused_level (the same for one level of the decimated search).
 //
 // What bounds the loop (measured with csrc/ubench_fp32.cu, profiles/r02_fp32_issue_rates.md): one warp instruction per
 // sub-partition per clock, a packed FADD2 / FMUL2 counts as two (it passes the 32-lane FMA pipe twice), an ALU-pipe
@@ -27,7 +28,9 @@
 //    The working layout INTERLEAVES them, float2 Z[i] = (yA[i], yB[i]), so that one packed FADD2 / FMUL2 advances one
 //    running sum of each sub-tile.
 //  * Each thread owns 8 consecutive samples of each sub-tile and keeps a sliding window of 8 float2 in registers
-//    (the width loop is unrolled by 8, so the rotation is register renaming): one LDS.64 per width step.
+//    (the width loop is unrolled by 8, so the rotation is register renaming): one LDS.128 per two width steps.
+//  * y is formed on the register pairs the 16-byte loads of the raw tile deliver (two consecutive samples of one
+//    sub-tile), the last step scalar, so the interleaved pairs need no register moves (Norm::apply_pair).
 //  * Samples past the row end are staged as -inf: a running sum that has touched one is -inf for every wider
 //    width, so "only widths that fit" (reading A9) needs no masking in the loop.  In the RC = false kernels widths
 //    nmax < w <= 8 ceil(nmax/8) get a NaN reciprocal: FMNMX drops NaN operands, so they can never win.
