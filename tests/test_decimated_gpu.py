@@ -202,3 +202,35 @@ def test_fused_decimated_config3_rows(P):
     x = gen.make_rows(cfg, rows)
     rec, info = _run_fused(P, x, 16, 4, "sqrt", O.stats(x), thr=cfg.threshold)
     assert info["gpu_hits"] > 0
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_random_decimated_cases_against_the_oracle(P, seed):
+    """Seeded random shapes / w0 / levels / sigma modes / row strides through both decimated paths (planes + candidate pass,
+    and the fused search); row lengths straddle the 1024-sample tiles (whole aligned tiles take the straight-line store path)."""
+    r = np.random.default_rng(1611 + seed)
+    done = 0
+    while done < 8:
+        n_dm = int(r.integers(1, 4))
+        n_t = int(r.choice([r.integers(40, 1200), r.integers(1200, 9000), 4096, 8192, 3072 + 4 * int(r.integers(0, 300))]))
+        w0 = int(r.choice([16, 32]))
+        if n_t < w0:
+            continue
+        lmax = 1
+        while lmax < 8 and (w0 << lmax) <= min(n_t, 4096):
+            lmax += 1
+        levels = int(r.integers(1, lmax + 1))
+        mode = str(r.choice(["sqrt", "sqrt", "linear", "anchored"]))
+        if n_dm * (n_t - (w0 << (levels - 1)) + 1) < 16:
+            mode = "sqrt"
+        mu, sg = float(r.choice([0.0, -50.0, 100.0])), float(r.choice([1.0, 0.1, 20.0]))
+        x = (mu + sg * r.standard_normal((n_dm, n_t))).astype(np.float32)
+        x[0, 20:20 + int(r.integers(1, min(30, n_t - 20)))] += 5 * sg
+        stride = None if r.random() < 0.6 else n_t + int(r.integers(1, 9))
+        thr = float(r.choice([3.0, 4.0, 5.0]))
+        try:
+            _run(P, x, w0, levels, mode, thr=thr, stride=stride)
+            _run_fused(P, x, w0, levels, mode, thr=thr, stride=stride)
+        except AssertionError as e:
+            raise AssertionError(f"seed {seed} case {done}: {n_dm}x{n_t} w0 {w0} levels {levels} {mode} mu {mu} sigma {sg} stride {stride} thr {thr}: {e}")
+        done += 1
