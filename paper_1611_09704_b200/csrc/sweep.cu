@@ -458,6 +458,9 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
     const float NINF = __int_as_float(0xff800000);
     const int mask7 = opaque_reg(~7);
     const bool row_tables = !RC && stats_stride != 0;
+    // every row of both planes 16-byte aligned: whole tiles take the straight-line store path
+    const bool planes_fast = ((reinterpret_cast<uintptr_t>(snr) & 15) == 0) && ((row_stride & 3) == 0) &&
+                             (width == nullptr || (((reinterpret_cast<uintptr_t>(width) & 15) == 0) && ((row_stride & 7) == 0)));
 
     if (!row_tables) for (int w = tid; w < sw_rt_len(nmax); w += SW_THREADS) rtf[w] = RC ? c_isqrt.v[w] : __ldg(table + w);
 
@@ -596,7 +599,20 @@ boxcar_snr_sweep(const float *__restrict__ x, int64_t n_t, int64_t row_stride, i
             for (int j = 0; j < SW_R; ++j) best[j] = make_float2(rtf[0], rtf[0]);
         }
 
-        store_planes<SW_THREADS>(snr, width, row, row_stride, n_t, T0 + SW_R * tid, best, wx, wy);
+        if (planes_fast && T0 + SW_TILE <= n_t) {             // whole tile inside 16-byte aligned planes: straight-line 16-byte streaming stores
+            float *oa = snr + row * row_stride + (T0 + SW_R * tid), *ob = oa + SW_SUB;
+            __stcs(reinterpret_cast<float4 *>(oa), make_float4(best[0].x, best[1].x, best[2].x, best[3].x));
+            __stcs(reinterpret_cast<float4 *>(oa) + 1, make_float4(best[4].x, best[5].x, best[6].x, best[7].x));
+            __stcs(reinterpret_cast<float4 *>(ob), make_float4(best[0].y, best[1].y, best[2].y, best[3].y));
+            __stcs(reinterpret_cast<float4 *>(ob) + 1, make_float4(best[4].y, best[5].y, best[6].y, best[7].y));
+            if (width) {
+                uint16_t *wa = width + row * row_stride + (T0 + SW_R * tid), *wb = wa + SW_SUB;
+                __stcs(reinterpret_cast<uint4 *>(wa), make_uint4(wx[0] | (wx[1] << 16), wx[2] | (wx[3] << 16), wx[4] | (wx[5] << 16), wx[6] | (wx[7] << 16)));
+                __stcs(reinterpret_cast<uint4 *>(wb), make_uint4(wy[0] | (wy[1] << 16), wy[2] | (wy[3] << 16), wy[4] | (wy[5] << 16), wy[6] | (wy[7] << 16)));
+            }
+        } else {
+            store_planes<SW_THREADS>(snr, width, row, row_stride, n_t, T0 + SW_R * tid, best, wx, wy);
+        }
     }
     cp_async_commit_wait_all();
 }
