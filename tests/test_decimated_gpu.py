@@ -234,3 +234,35 @@ def test_random_decimated_cases_against_the_oracle(P, seed):
         except AssertionError as e:
             raise AssertionError(f"seed {seed} case {done}: {n_dm}x{n_t} w0 {w0} levels {levels} {mode} mu {mu} sigma {sg} stride {stride} thr {thr}: {e}")
         done += 1
+
+
+def test_fused_decimated_search_is_cuda_graph_capturable(P):
+    """spd_stats + spd_search_fused_decimated only enqueue work on the caller's stream and keep no state: captured once,
+    replayed with the same result."""
+    cfg = gen.get_config(1)
+    x = torch.from_numpy(gen.make_array(cfg)).cuda()
+    st, ws = P.new_stats("cuda"), P.new_workspace(cfg.n_dm, cfg.n_t, 32, "cuda")
+    dws = torch.empty(int(P.lib().spd_decimated_workspace_bytes(cfg.n_dm, cfg.n_t, 16, 2)), dtype=torch.uint8, device="cuda")
+    out, cnt = P.new_candidates(4096, "cuda")
+
+    def step():
+        P.spd_stats(x, 0, st, ws)
+        P.spd_search_fused_decimated(x, st, 16, 2, "sqrt", cfg.threshold, out, cnt, ws=dws)
+
+    step()
+    torch.cuda.synchronize()
+    n0 = int(cnt.item())
+    ref = np.sort(out[:n0].cpu().numpy().view(P.CAND_DTYPE).reshape(-1), order=["dm", "t", "width"])
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        step()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            step()
+    torch.cuda.synchronize()
+    cnt.zero_(); out.zero_(); st.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert int(cnt.item()) == n0 > 0
+    got = np.sort(out[:n0].cpu().numpy().view(P.CAND_DTYPE).reshape(-1), order=["dm", "t", "width"])
+    assert got.tobytes() == ref.tobytes()
