@@ -1,8 +1,8 @@
 """Chunked streaming with copy / compute overlap (the real-time pipeline shape of PAPER.md:97).
 
 A telescope back-end produces one de-dispersed chunk [n_dm][n_t] after another.  `ChunkStream` keeps `depth` device
-slots; the host-to-device copy of chunk i+1 runs on a copy stream while spd_stats + spd_search_fused of chunk i run on
-a compute stream, and the statistics, the hit count and the records of a finished chunk come back through pinned host
+slots; the host-to-device copy of chunk i+1 runs on a copy stream while spd_stats + spd_search_fused (or, on request,
+spd_search_fused_decimated) of chunk i run on a compute stream, and the statistics, the hit count and the records of a finished chunk come back through pinned host
 buffers.  This module is plumbing only (CUDA streams and events from PyTorch, argument marshalling); every step of
 the search runs in the kernels behind the C ABI.
 
@@ -38,10 +38,18 @@ def time_chunks(n_total: int, chunk_len: int, nmax: int) -> List[Tuple[int, int,
 
 class ChunkStream:
     def __init__(self, n_dm: int, n_t: int, nmax: int, mode="sqrt", threshold: float = 6.0, capacity: int = 1 << 20,
-                 depth: int = 2, device="cuda"):
+                 depth: int = 2, device="cuda", decimated: Optional[Tuple[int, int]] = None):
+        """decimated = (w0, levels): search every chunk with spd_search_fused_decimated (nmax must equal
+        w0 * 2^(levels-1)) instead of the exhaustive spd_search_fused."""
         if depth < 1:
             raise ValueError("depth >= 1")
         B.lib()
+        self.decimated = None
+        if decimated is not None:
+            w0, levels = int(decimated[0]), int(decimated[1])
+            if nmax != w0 << (levels - 1) or int(B.lib().spd_decimated_workspace_bytes(n_dm, n_t, w0, levels)) == 0:
+                raise B.SpdError("ChunkStream: decimated = (w0, levels) needs w0 in {16, 32}, nmax == w0 * 2^(levels-1) <= 4096")
+            self.decimated = (w0, levels)
         self.n_dm, self.n_t, self.nmax, self.mode, self.threshold, self.capacity = n_dm, n_t, int(nmax), mode, float(threshold), int(capacity)
         self.dev = torch.device(device)
         self.copy_stream = torch.cuda.Stream(self.dev)
@@ -53,6 +61,8 @@ class ChunkStream:
             self.slots.append({
                 "x": torch.empty((n_dm, n_t), dtype=torch.float32, device=self.dev),
                 "stats": B.new_stats(self.dev), "ws": B.new_workspace(n_dm, n_t, self.nmax, self.dev),
+                "dws": None if self.decimated is None else torch.empty(
+                    int(B.lib().spd_decimated_workspace_bytes(n_dm, n_t, *self.decimated)), dtype=torch.uint8, device=self.dev),
                 "out": out, "cnt": cnt,
                 "h_out": torch.zeros((self.capacity, 4), dtype=torch.int32).pin_memory(),
                 "h_cnt": torch.zeros(1, dtype=torch.int64).pin_memory(),
@@ -82,8 +92,12 @@ class ChunkStream:
                 B.spd_stats(s["x"], self.nsig, s["stats"], s["ws"], stream=self.compute_stream)
             else:
                 s["stats"].copy_(stats, non_blocking=True)
-            B.spd_search_fused(s["x"], s["stats"], self.nmax, self.mode, self.threshold, s["out"], s["cnt"], ws=s["ws"],
-                               stream=self.compute_stream)
+            if self.decimated is None:
+                B.spd_search_fused(s["x"], s["stats"], self.nmax, self.mode, self.threshold, s["out"], s["cnt"], ws=s["ws"],
+                                   stream=self.compute_stream)
+            else:
+                B.spd_search_fused_decimated(s["x"], s["stats"], self.decimated[0], self.decimated[1], self.mode, self.threshold,
+                                             s["out"], s["cnt"], ws=s["dws"], stream=self.compute_stream)
             s["h_cnt"].copy_(s["cnt"], non_blocking=True)
             s["h_stats"].copy_(s["stats"], non_blocking=True)
             s["h_out"].copy_(s["out"], non_blocking=True)          # whole buffer: the count is not known on the host yet

@@ -99,3 +99,21 @@ def test_chunk_stream_refuses_to_overrun_its_slots(P):
     assert int(st["n"][0]) == 4 * 2048
     with pytest.raises(P.SpdError):
         cs.result(t)
+
+
+def test_chunk_stream_with_the_decimated_search_equals_the_oracle(P):
+    """ChunkStream(decimated=(16, 3)): every chunk's list is the ORACLE's decimated candidate list (O5 + O4) of that chunk."""
+    from oracle import spd_oracle as O
+    from oracle import compare as CMP
+    from paper_1611_09704_b200.stream import ChunkStream
+    base = gen.get_config(1)
+    chunks = [gen.make_array(dataclasses.replace(base, cid=base.cid + 100 * k)) for k in range(3)]
+    cs = ChunkStream(base.n_dm, base.n_t, 64, "sqrt", base.threshold, capacity=1 << 14, depth=2, decimated=(16, 3))
+    got = cs.run([torch.from_numpy(c).pin_memory() for c in chunks])
+    for x, (rec, total) in zip(chunks, got):
+        o = O.search_decimated(x, 16, 3, "sqrt", base.threshold)
+        r = CMP.compare_candidates_decimated(rec["dm"], rec["t"], rec["snr"], rec["width"], total, 1 << 14, o["levels"], 16, base.threshold,
+                                             x, o["stats"].mean, o["sig"])
+        assert r and total > 0, str(r)
+    with pytest.raises(P.SpdError):
+        ChunkStream(base.n_dm, base.n_t, 100, "sqrt", base.threshold, decimated=(16, 3))      # nmax != w0 * 2^(levels-1)
