@@ -54,7 +54,8 @@ def test_stats_parity(P, shape, mu, sigma, stride):
 
 
 @pytest.mark.parametrize("shape,nmax", [((4, 100), 1), ((4, 100), 16), ((3, 5000), 512), ((2, 9000), 100), ((1, 64), 64),
-                                        ((9, 4200), 33)])
+                                        ((9, 4200), 33), ((2, 20000), 4096), ((1, 4096), 4096), ((3, 12288), 15), ((3, 12288), 17),
+                                        ((2, 8192 + 2047), 2048), ((5, 16384), 4080), ((2, 4097), 31)])
 def test_sigma_nmax_parity(P, shape, nmax):
     from gpu_util import gpu_stats
     x = (1.0 + rng(101).standard_normal(shape)).astype(np.float32)
