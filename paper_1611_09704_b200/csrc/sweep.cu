@@ -1127,6 +1127,8 @@ cudaError_t launch_sweep(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
                          bool fused, float threshold, spd_candidate_t *out, unsigned long long capacity,
                          unsigned long long *d_count, cudaStream_t s, int stats_stride)
 {
+    if (fused && stats_stride == 0 && nmax <= 32 && (nmax & 7) == 0)        // narrow fused search: the straight-line level kernel (level 0, scale 1)
+        return launch_search_level(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, 0, 1, rc, threshold, out, capacity, d_count, nullptr, 0, s);
     if (!fused && nmax > SW_NARROW_NMAX && nmax <= SW_WARP_CTA_NMAX) {       // general plane kernel, one-warp CTAs
         if (rc) return launch_sweep_nt<32, true>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s, stats_stride);
         return launch_sweep_nt<32, false>(x, n_dm, n_t, row_stride, d_stats, d_table, nmax, snr, width, fused, threshold, out, capacity, d_count, s, stats_stride);
@@ -1186,8 +1188,10 @@ cudaError_t launch_search_level(const float *xl, int64_t n_dm, int64_t n_l, int6
                                 unsigned long long capacity, unsigned long long *d_count, float *dec_out, int64_t dec_stride, cudaStream_t s)
 {
     if (n_l <= 0) return cudaSuccess;
-    if ((w0 != 16 && w0 != 32) || (wmin != 0 && wmin != w0 / 2)) return cudaErrorInvalidValue;
+    if (w0 < 8 || w0 > 32 || (w0 & 7) || (wmin != 0 && (wmin != w0 / 2 || (w0 & 15)))) return cudaErrorInvalidValue;
 #define SPD_LEVEL(RC_, W0_, L0_) launch_search_level_t<RC_, W0_, L0_>(xl, n_dm, n_l, xl_stride, d_stats_level, d_table, wscale, threshold, out, capacity, d_count, dec_out, dec_stride, s)
+    if (w0 == 8) return rc ? SPD_LEVEL(true, 8, true) : SPD_LEVEL(false, 8, true);            // (exhaustive fused search at Nmax 8 / 24)
+    if (w0 == 24) return rc ? SPD_LEVEL(true, 24, true) : SPD_LEVEL(false, 24, true);
     if (w0 == 16) {
         if (wmin == 0) return rc ? SPD_LEVEL(true, 16, true) : SPD_LEVEL(false, 16, true);
         return rc ? SPD_LEVEL(true, 16, false) : SPD_LEVEL(false, 16, false);
