@@ -348,8 +348,20 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
     float y[ST_RUN];
 #pragma unroll
     for (int k = 0; k < ST_RUN; ++k) y[k] = (FAST || k < cnt) ? xo[k] - K : 0.f;
-    const float rt = (((y[0] + y[1]) + (y[2] + y[3])) + ((y[4] + y[5]) + (y[6] + y[7]))) +
-                     (((y[8] + y[9]) + (y[10] + y[11])) + ((y[12] + y[13]) + (y[14] + y[15])));
+    // ---- sample statistics of the tile's own 4096 positions (eq. 1 per run, eq. 2 into the lane's partial); the run total
+    //      rt = sum of y is eq. 1's own T ----
+    float rt;
+    if (FAST || cnt == ST_RUN) {
+        float T, S;
+        chan_run16(y, T, S);
+        rt = T;
+        L.push_run(T, S);
+    } else {
+        const Tri t = chan_run_ragged(y, cnt);
+        rt = (float)t.T;
+        L.flush();
+        tri_merge(L.acc, t);
+    }
     const bool hwarp = 32 * wid < nh + 1;                      // warp-uniform: this warp holds halo runs (or the entry after the last)
     float ht = 0.f;
     if (tid < nh) {                                            // thread tid sums halo run tid
@@ -361,17 +373,6 @@ __device__ __forceinline__ void win_tile(const float *__restrict__ xs, float *__
     float inc = rt, inch = ht;
     if (hwarp) warp_scan_incl2(inc, inch); else inc = warp_scan_incl(inc);
     if (lane == 31) { wtot[0][wid] = inc; wtot[1][wid] = inch; mbar_arrive(mbar); }      // 8 arrivals complete the phase
-
-    // ---- sample statistics of the tile's own 4096 positions (eq. 1 per run, eq. 2 into the lane's partial) ----
-    if (FAST || cnt == ST_RUN) {
-        float T, S;
-        chan_run16(y, T, S);
-        L.push_run(T, S);
-    } else {
-        const Tri t = chan_run_ragged(y, cnt);
-        L.flush();
-        tri_merge(L.acc, t);
-    }
 
     // ---- exclusive prefix Q of the run totals: the tile's 256 runs, then the nh halo runs ----
     mbar_wait(mbar, parity);
