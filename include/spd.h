@@ -26,7 +26,9 @@
 extern "C" {
 #endif
 
-typedef enum { SPD_OK = 0, SPD_ERR_INVALID_ARG = 1, SPD_ERR_CUDA = 2, SPD_ERR_WORKSPACE = 3 } spd_status;
+typedef enum { SPD_OK = 0, SPD_ERR_INVALID_ARG = 1, SPD_ERR_CUDA = 2, SPD_ERR_WORKSPACE = 3,
+               SPD_ERR_NOALLOC_LIMIT = 4   /* spd_stats_rows_noalloc only: more rows than its built-in scratch holds */
+} spd_status;
 
 /* sigma after an N-sample boxcar (section 2.2) */
 typedef enum {
@@ -129,6 +131,30 @@ spd_status spd_search_fused_rows(const float *d_x, int64_t n_dm, int64_t n_t, in
                                  const spd_stats_t *d_stats_rows, int nmax, spd_sigma_mode mode, float threshold,
                                  spd_candidate_t *d_out, uint64_t capacity, unsigned long long *d_count,
                                  void *d_ws, size_t ws_bytes, void *stream);
+
+/* spd_stats_rows for callers that cannot obtain device memory of their own.
+ * Who that is: a detection stage running inside somebody else's real-time pipeline.  The host framework owns the card: it
+ * has split the whole of device memory into its own pools at start-up, passes each stage the device buffers it reads and
+ * writes, and does not let a stage call cudaMalloc (the memory is already spoken for, and an allocation makes the device
+ * wait, which would stall the other stages' streams mid-observation).  Such a caller has its input and its result buffer,
+ * but nowhere to put the workspace spd_stats_rows needs.  Here the workspace is a fixed array inside libspd.so instead.
+ *
+ * Same arguments, kernels and results as spd_stats_rows (bit for bit), minus d_ws / ws_bytes.  d_x and d_stats_rows are
+ * still the caller's.  The call allocates nothing: no cudaMalloc / cudaFree and no library routine that allocates.
+ * Limit: n_dm <= SPD_NOALLOC_MAX_ROWS (8192; spd_stats_rows_noalloc_max_rows() returns it).  More rows than that return
+ * SPD_ERR_NOALLOC_LIMIT before anything is launched: split the rows over several calls, one after the other on one stream.
+ * Cost: the array is 3 MiB (8192 rows x 8 partials x 2 x 24 bytes) of device memory on EVERY GPU that loads the library,
+ * held until the process exits, also by programs that never call this.
+ * First call on a device: it looks up the array's device address (cudaGetSymbolAddress) and remembers it, with that device
+ * current; make that first call during start-up, before any stream capture begins.  Later calls only enqueue kernels.
+ * Shared state: all calls on one device use the same array.  It still holds the previous call's partials; nothing needs
+ * clearing, because a call overwrites every slot it later reads.  Two calls that can overlap on the GPU (different streams
+ * without an ordering between them, or two host threads on different streams) race on the array and give wrong statistics:
+ * keep calls on one stream, or order them with events.  This is the one entry point of the library that keeps state. */
+#define SPD_NOALLOC_MAX_ROWS 8192
+int64_t spd_stats_rows_noalloc_max_rows(void);
+spd_status spd_stats_rows_noalloc(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
+                                  spd_stats_t *d_stats_rows, void *stream);
 
 /* Decimation in time + boxcar for wide filters (section 3: "a combination of boxcar filtering with the
  * decimation in time of the input data"; the paper names the route, the algorithm is reading A20 of DESIGN.md).

@@ -54,6 +54,8 @@ def lib() -> C.CDLL:
         L.spd_search_host.argtypes = [vp, i64, i64, i32, i32, f32, vp, u64, vp, vp, vp, sz, vp]
         L.spd_workspace_bytes_rows.argtypes = [i64, i64, i32]; L.spd_workspace_bytes_rows.restype = sz
         L.spd_stats_rows.argtypes = [vp, i64, i64, i64, i32, vp, vp, sz, vp]
+        L.spd_stats_rows_noalloc.argtypes = [vp, i64, i64, i64, i32, vp, vp]
+        L.spd_stats_rows_noalloc_max_rows.argtypes = []; L.spd_stats_rows_noalloc_max_rows.restype = i64
         L.spd_boxcar_snr_rows.argtypes = [vp, i64, i64, i64, vp, i32, i32, vp, vp, vp, sz, vp]
         L.spd_search_fused_rows.argtypes = [vp, i64, i64, i64, vp, i32, i32, f32, vp, u64, vp, vp, sz, vp]
         L.spd_decimated_level_offset.argtypes = [i64, i32]; L.spd_decimated_level_offset.restype = i64
@@ -63,7 +65,7 @@ def lib() -> C.CDLL:
         L.spd_search_fused_decimated.argtypes = [vp, i64, i64, i64, vp, i32, i32, i32, f32, vp, u64, vp, vp, sz, vp]
         for f in ("spd_stats", "spd_stats_merge", "spd_boxcar_snr", "spd_candidates", "spd_search_fused", "spd_search_host",
                   "spd_boxcar_snr_decimated", "spd_candidates_decimated", "spd_search_fused_decimated", "spd_stats_rows", "spd_boxcar_snr_rows",
-                  "spd_search_fused_rows"):
+                  "spd_search_fused_rows", "spd_stats_rows_noalloc"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -185,6 +187,28 @@ def spd_stats_rows(x: torch.Tensor, nmax_for_sigma: int = 0, stats: Optional[tor
     _check(lib().spd_stats_rows(x.data_ptr(), n_dm, n_t, rs, int(nmax_for_sigma), stats.data_ptr(), ws.data_ptr(), ws.numel(),
                                 _stream(stream)), "spd_stats_rows")
     return stats
+
+
+def spd_stats_rows_noalloc(x: torch.Tensor, stats: torch.Tensor, nmax_for_sigma: int = 0, stream=None) -> torch.Tensor:
+    """spd_stats_rows for code that may not allocate device memory: a stage inside a real-time pipeline whose host
+    framework owns every byte of the card and hands the stage its input and output buffers, nothing else.
+
+    `x` and `stats` (uint8[n_dm * 80], e.g. a slice of the framework's output buffer) are the caller's; the workspace
+    that spd_stats_rows would need is a 3 MiB array inside libspd.so.  Neither this function nor the C call behind it
+    allocates.  At most noalloc_max_rows() = 8192 rows per call: more raises SpdError (SPD_ERR_NOALLOC_LIMIT) and
+    launches nothing.  Results equal spd_stats_rows bit for bit.  Calls share the array, so issue them on one stream
+    (or order them with events): calls that overlap on the GPU corrupt each other's statistics.  Make the first call on
+    each device during start-up; it resolves the array's device address."""
+    n_dm, n_t, rs = _plane(x, torch.float32, "x")
+    if stats.device != x.device or stats.dtype != torch.uint8 or not stats.is_contiguous() or stats.numel() < n_dm * STATS_BYTES:
+        raise SpdError("stats must be a contiguous uint8 tensor of n_dm * 80 bytes on x's device")
+    _check(lib().spd_stats_rows_noalloc(x.data_ptr(), n_dm, n_t, rs, int(nmax_for_sigma), stats.data_ptr(), _stream(stream)),
+           "spd_stats_rows_noalloc")
+    return stats
+
+
+def noalloc_max_rows() -> int:
+    return int(lib().spd_stats_rows_noalloc_max_rows())
 
 
 def spd_boxcar_snr_rows(x: torch.Tensor, stats_rows: torch.Tensor, nmax: int, mode="sqrt",

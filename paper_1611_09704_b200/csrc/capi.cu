@@ -26,6 +26,7 @@ const char *spd_status_string(spd_status s)
     case SPD_ERR_INVALID_ARG: return "SPD_ERR_INVALID_ARG";
     case SPD_ERR_CUDA: return "SPD_ERR_CUDA";
     case SPD_ERR_WORKSPACE: return "SPD_ERR_WORKSPACE";
+    case SPD_ERR_NOALLOC_LIMIT: return "SPD_ERR_NOALLOC_LIMIT: n_dm exceeds SPD_NOALLOC_MAX_ROWS (8192 rows per spd_stats_rows_noalloc call)";
     }
     return "SPD_ERR_UNKNOWN";
 }
@@ -123,6 +124,20 @@ spd_status spd_stats_rows(const float *d_x, int64_t n_dm, int64_t n_t, int64_t r
     if ((reinterpret_cast<uintptr_t>(d_ws) & 15) != 0) return SPD_ERR_INVALID_ARG;
     if (ws_bytes < stats_rows_ws_bytes(n_dm)) return SPD_ERR_WORKSPACE;
     cudaError_t e = launch_stats_rows(d_x, n_dm, n_t, row_stride, nmax_for_sigma, d_stats_rows, d_ws, (cudaStream_t)stream);
+    return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
+}
+
+// spd_stats_rows without a caller workspace: the block partials go to a static device array in stats.cu (see spd.h for
+// who needs this and what it costs).  No allocation here or below; too many rows are refused before any launch.
+int64_t spd_stats_rows_noalloc_max_rows(void) { return SPD_NOALLOC_MAX_ROWS; }
+
+spd_status spd_stats_rows_noalloc(const float *d_x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
+                                  spd_stats_t *d_stats_rows, void *stream)
+{
+    if (!d_x || !d_stats_rows || !shape_ok(n_dm, n_t, row_stride)) return SPD_ERR_INVALID_ARG;
+    if (nmax_for_sigma < 0 || (nmax_for_sigma > 0 && !nmax_ok(nmax_for_sigma, n_t))) return SPD_ERR_INVALID_ARG;
+    if (n_dm > SPD_NOALLOC_MAX_ROWS) return SPD_ERR_NOALLOC_LIMIT;
+    cudaError_t e = launch_stats_rows_noalloc(d_x, n_dm, n_t, row_stride, nmax_for_sigma, d_stats_rows, (cudaStream_t)stream);
     return e == cudaSuccess ? SPD_OK : SPD_ERR_CUDA;
 }
 

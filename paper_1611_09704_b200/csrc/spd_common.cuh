@@ -44,6 +44,8 @@ cudaError_t launch_stats(const float *x, int64_t n_dm, int64_t n_t, int64_t row_
 cudaError_t launch_stats_rows(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
                               spd_stats_t *d_stats_rows, void *d_ws, cudaStream_t s);
 size_t stats_rows_ws_bytes(int64_t n_dm);
+cudaError_t launch_stats_rows_noalloc(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
+                                      spd_stats_t *d_stats_rows, cudaStream_t s);     // partials in the library's own static array
 cudaError_t launch_stats_merge(const spd_stats_t *parts, int count, spd_stats_t *out, cudaStream_t s);
 cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, float *d_table, cudaStream_t s,
                                int wscale = 1, int nmax_total = 0, int64_t rows = 1);

@@ -686,6 +686,50 @@ cudaError_t launch_stats_rows(const float *x, int64_t n_dm, int64_t n_t, int64_t
     return cudaGetLastError();
 }
 
+// ---- spd_stats_rows_noalloc: the per-row statistics with the block partials in memory the library itself owns ----
+// Some users of this library run where device memory cannot be requested at all: a search stage plugged into a
+// telescope's real-time pipeline is handed its input and output buffers by the host framework, which has already
+// carved the whole card into its own pools and forbids stages to allocate (an allocation would also stall every other
+// stage: cudaMalloc waits for the device).  Such a caller has no way to produce the workspace spd_stats_rows asks for.
+// For them the partials live in this file-scope array instead: 3 MiB that every GPU which loads libspd.so holds until
+// the process exits, whether or not this entry point is ever called.
+//
+// In host code `noalloc_scratch` is only a handle for the symbol, never a device address (a kernel handed it would fault,
+// or, on a GPU that can reach host memory, quietly work on the wrong bytes).  The address on the current device comes
+// from cudaGetSymbolAddress, looked up once per device and remembered.
+constexpr size_t NOALLOC_SCRATCH_BYTES = (size_t)SPD_NOALLOC_MAX_ROWS * ST_ROW_CTAS * 2 * sizeof(Tri);
+static __device__ __align__(256) unsigned char noalloc_scratch[NOALLOC_SCRATCH_BYTES];
+
+static cudaError_t noalloc_scratch_address(void **out)
+{
+    static std::mutex mu;
+    static void *known[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lk(mu);
+    if (dev >= 0 && dev < 64 && known[dev]) { *out = known[dev]; return cudaSuccess; }
+    void *p = nullptr;
+    if ((e = cudaGetSymbolAddress(&p, noalloc_scratch)) != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    if (dev >= 0 && dev < 64) known[dev] = p;
+    *out = p;
+    return cudaSuccess;
+}
+
+// Same kernels, grid and partial layout as launch_stats_rows; only where the partials live differs.  Nothing in the
+// array has to be cleared between calls: every CTA stores its partial before the finalize kernel of the same call reads
+// it, and slots beyond this call's n_dm * gx are never read.
+cudaError_t launch_stats_rows_noalloc(const float *x, int64_t n_dm, int64_t n_t, int64_t row_stride, int nmax_for_sigma,
+                                      spd_stats_t *d_stats_rows, cudaStream_t s)
+{
+    if (stats_rows_ws_bytes(n_dm) > NOALLOC_SCRATCH_BYTES) return cudaErrorInvalidValue;   // the C ABI has already refused it
+    void *scratch = nullptr;
+    cudaError_t e = noalloc_scratch_address(&scratch);
+    if (e != cudaSuccess) return e;
+    return launch_stats_rows(x, n_dm, n_t, row_stride, nmax_for_sigma, d_stats_rows, scratch, s);
+}
+
 cudaError_t launch_stats_merge(const spd_stats_t *parts, int count, spd_stats_t *out, cudaStream_t s)
 {
     stats_merge_kernel<<<1, 32, 0, s>>>(parts, count, out);
