@@ -300,11 +300,17 @@ def spd_search_fused_decimated(x: torch.Tensor, stats: torch.Tensor, w0: int, le
     return out, count
 
 
+def check_count(total: int) -> int:
+    """The hit count as read into an int64: -1 is 0xFFFFFFFFFFFFFFFF, the 'sigma_N undefined' sentinel of spd_search_fused /
+    spd_search_fused_decimated (include/spd.h): no record was written, so there is no list to hand back."""
+    if total < 0:
+        raise SpdError("spd_search_fused: sigma_N is undefined (a LINEAR mode fed statistics measured for another Nmax)")
+    return total
+
+
 def read_candidates(out: torch.Tensor, count: torch.Tensor) -> Tuple[np.ndarray, int]:
     """Device list -> (numpy structured array of the written records, total hit count).  Synchronises."""
-    total = int(count.item())
-    if total < 0:      # 0xFFFFFFFFFFFFFFFF: spd_search_fused was fed a NaN sigma table (include/spd.h)
-        raise SpdError("spd_search_fused: sigma_N is undefined (a LINEAR mode fed statistics measured for another Nmax)")
+    total = check_count(int(count.item()))
     got = min(total, out.shape[0])
     rec = out[:got].cpu().numpy().view(CAND_DTYPE).reshape(-1)
     return rec, total
