@@ -10,6 +10,10 @@ Chunks along TIME for the same DM trials must overlap by Nmax - 1 samples: the l
 the widths that fit (reading A9), so the next chunk starts Nmax - 1 samples before the end of this one and the
 records of those last Nmax - 1 start samples are dropped from every chunk but the last (`time_chunks`,
 `ChunkStream.run_time_axis`): every start sample of the series is then searched exactly once with every width.
+With the decimated search the chunk starts must also be multiples of 2^(levels-1), or the pair sums of a later chunk
+would straddle the pairs of the series' own decimation: `time_chunks(..., align=2^(levels-1))` rounds the step down
+(the overlap grows by up to 2^(levels-1) - 1 samples) and the union of the records is then the decimated search of the
+whole series, level grid for level grid.
 """
 from __future__ import annotations
 
@@ -21,12 +25,15 @@ import torch
 from . import binding as B
 
 
-def time_chunks(n_total: int, chunk_len: int, nmax: int) -> List[Tuple[int, int, int]]:
-    """Cut a time axis of n_total samples into chunks of <= chunk_len samples that overlap by nmax - 1:
-    [(start, length, keep)]; records with local start sample t < keep belong to the chunk (all of them in the last one)."""
-    if not (1 <= nmax <= chunk_len and n_total >= 1):
-        raise ValueError("time_chunks: need 1 <= nmax <= chunk_len and n_total >= 1")
-    out, s, step = [], 0, chunk_len - (nmax - 1)
+def time_chunks(n_total: int, chunk_len: int, nmax: int, align: int = 1) -> List[Tuple[int, int, int]]:
+    """Cut a time axis of n_total samples into chunks of <= chunk_len samples that overlap by at least nmax - 1:
+    [(start, length, keep)]; records with local start sample t < keep belong to the chunk (all of them in the last one).
+    Every start is a multiple of `align` (2^(levels-1) for the decimated search; 1 for the exhaustive one)."""
+    if not (1 <= nmax <= chunk_len and n_total >= 1 and align >= 1):
+        raise ValueError("time_chunks: need 1 <= nmax <= chunk_len, n_total >= 1 and align >= 1")
+    out, s, step = [], 0, (chunk_len - (nmax - 1)) // align * align
+    if step < 1:
+        raise ValueError("time_chunks: chunk_len - nmax + 1 is shorter than one aligned step")
     while True:
         length = min(chunk_len, n_total - s)
         last = s + length >= n_total
@@ -113,7 +120,7 @@ class ChunkStream:
             raise B.SpdError("ChunkStream: no chunk in flight in this slot")
         s["done"].synchronize()
         s["busy"] = False
-        total = int(s["h_cnt"][0])
+        total = B.check_count(int(s["h_cnt"][0]))      # raises on the 'sigma_N undefined' sentinel (stats of another Nmax)
         got = min(total, self.capacity)
         rec = s["h_out"][:got].numpy().view(B.CAND_DTYPE).reshape(-1)
         return rec, total, s["h_stats"].numpy().view(B.STATS_DTYPE)
@@ -121,11 +128,14 @@ class ChunkStream:
     def run_time_axis(self, h_series: torch.Tensor, stats: Optional[torch.Tensor] = None) -> Tuple[np.ndarray, int]:
         """Search a long series [n_dm][T] (pinned CPU tensor) as consecutive chunks of the stream's n_t samples that
         overlap by nmax - 1; returns (records with t in samples of the SERIES, number of records).  The last chunk must
-        have the stream's length too: T = n_t + k (n_t - nmax + 1)."""
+        have the stream's length too: T = n_t + k step, step = n_t - nmax + 1 (decimated stream: rounded down to a
+        multiple of 2^(levels-1) so that every chunk's level grids are the series' own; the result is then the
+        decimated search of the whole series)."""
         T = h_series.shape[1]
-        plan = time_chunks(T, self.n_t, self.nmax)
+        align = 1 if self.decimated is None else 1 << (self.decimated[1] - 1)
+        plan = time_chunks(T, self.n_t, self.nmax, align)
         if any(length != self.n_t for _, length, _ in plan):
-            raise B.SpdError("run_time_axis: the series length must be n_t + k (n_t - nmax + 1)")
+            raise B.SpdError(f"run_time_axis: the series length must be n_t + k * {(self.n_t - self.nmax + 1) // align * align}")
         recs: List[np.ndarray] = []
         tickets: List[Tuple[int, int, int]] = []
 

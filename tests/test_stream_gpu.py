@@ -117,3 +117,57 @@ def test_chunk_stream_with_the_decimated_search_equals_the_oracle(P):
         assert r and total > 0, str(r)
     with pytest.raises(P.SpdError):
         ChunkStream(base.n_dm, base.n_t, 100, "sqrt", base.threshold, decimated=(16, 3))      # nmax != w0 * 2^(levels-1)
+
+
+def test_chunk_stream_result_raises_on_statistics_of_another_nmax(P):
+    """LINEAR-mode statistics measured for another Nmax leave sigma_N undefined: the search writes the UINT64_MAX sentinel
+    instead of a count (include/spd.h), and result() / run_time_axis must raise instead of handing back stale records."""
+    from paper_1611_09704_b200.stream import ChunkStream
+    n_dm, n_t, nmax = 4, 4096, 32
+    rng = np.random.Generator(np.random.PCG64(77))
+    x = torch.from_numpy(rng.standard_normal((n_dm, n_t)).astype(np.float32)).pin_memory()
+    wrong = P.write_stats(0.0, 1.0, 4.0, 16)                 # sigma_Nmax of Nmax 16, searched with Nmax 32
+    for dec in (None, (16, 2)):
+        cs = ChunkStream(n_dm, n_t, nmax, "linear", 5.0, capacity=256, depth=2, decimated=dec)
+        t = cs.submit(x, stats=wrong)
+        with pytest.raises(P.SpdError, match="sigma_N is undefined"):
+            cs.result(t)
+        with pytest.raises(P.SpdError, match="sigma_N is undefined"):
+            cs.run_time_axis(x, wrong)
+        right = P.write_stats(0.0, 1.0, float(np.sqrt(nmax)), nmax)
+        rec, total, _ = cs.result(cs.submit(x, stats=right))       # the stream is usable afterwards
+        assert total >= 0 and rec.size == min(total, 256)
+
+
+@pytest.mark.parametrize("mode,w0,levels", [("sqrt", 16, 3), ("anchored", 16, 4), ("sqrt", 32, 2)])
+def test_time_axis_chunks_of_a_decimated_stream_equal_the_oracle_on_the_whole_series(P, mode, w0, levels):
+    """run_time_axis on ChunkStream(decimated=...): chunk starts are multiples of 2^(levels-1), so each chunk's level grids
+    are the series' own and the union of the records is the ORACLE's decimated candidate list of the concatenated series
+    (reading A20)."""
+    from oracle import spd_oracle as O
+    from oracle import compare as CMP
+    from paper_1611_09704_b200.stream import ChunkStream, time_chunks
+    nmax = w0 << (levels - 1)
+    n_dm, n_t, k = 3, 4096, 3
+    G = 1 << (levels - 1)
+    step = (n_t - nmax + 1) // G * G
+    assert step != n_t - nmax + 1                           # the unaligned step would shift the level grids
+    T = n_t + k * step
+    rng = np.random.Generator(np.random.PCG64(950 + nmax))
+    x = (2.0 + 1.5 * rng.standard_normal((n_dm, T))).astype(np.float32)
+    for c in range(1, k + 1):                               # pulses straddling every chunk boundary, and one at the very end
+        b = c * step
+        x[c % n_dm, b - nmax // 2:b + nmax // 3] += 1.5
+    x[0, T - 20:] += 4.0
+    thr = 5.0
+    o = O.search_decimated(x, w0, levels, mode, thr)
+    st = o["stats"]
+    plan = time_chunks(T, n_t, nmax, G)
+    assert all(s % G == 0 and length == n_t for s, length, _ in plan) and len(plan) == k + 1
+    d_st = P.write_stats(st.mean, st.sigma, st.sigma_nmax, st.nmax_of_sigma)
+    cs = ChunkStream(n_dm, n_t, nmax, mode, thr, capacity=1 << 16, depth=2, decimated=(w0, levels))
+    rec, total = cs.run_time_axis(torch.from_numpy(x).pin_memory(), d_st)
+    r = CMP.compare_candidates_decimated(rec["dm"], rec["t"], rec["snr"], rec["width"], total, 1 << 16, o["levels"], w0, thr,
+                                         x, st.mean, o["sig"])
+    assert r and total > 50, str(r)
+    assert (rec["t"] >= T - 20).any() and (rec["width"] > w0).any()
