@@ -246,9 +246,10 @@ def extra_legs(torch, P, args, dev, step, barrier, d_x, h_x, st, ws, out, cnt, a
     barrier()
     ms_pipe = p0.elapsed_time(p1) / pipe_steps
     hits_pipe = pipe_res[-1][1]
+    d2h_pipe = cs.bytes_d2h                             # what the last chunk actually moved back (count + stats + records)
     del cs
 
-    return graph_ms, fused_ms, fused_kernel_ms, hits_fused, ms_e2e, hits_e2e, e2e_steps, ms_pipe, hits_pipe, pipe_steps
+    return graph_ms, fused_ms, fused_kernel_ms, hits_fused, ms_e2e, hits_e2e, e2e_steps, ms_pipe, hits_pipe, pipe_steps, d2h_pipe
 
 
 def decimated_leg(torch, P, args, d_x, st, ws, n_dm, n_t, nmax, nmax_sigma, mode, thr, cap, hbm_peak):
@@ -415,7 +416,7 @@ def run_ours(args):
     extras = not shard_rows and not args.no_e2e
     graph_ms = fused_ms = fused_kernel_ms = ms_e2e = ms_pipe = float("nan")
     hits_fused = hits_e2e = hits_pipe = -1
-    e2e_steps = pipe_steps = 0
+    e2e_steps = pipe_steps = d2h_pipe = 0
     if shard_rows and not args.no_e2e:
         # end to end for the sharded run: H2D of the rank's rows from pinned memory, shard.sharded_search (fused), D2H of count + records
         h_out = torch.zeros((cap, 4), dtype=torch.int32).pin_memory()
@@ -431,7 +432,7 @@ def run_ours(args):
         f1.record(); barrier()
         ms_e2e = f0.elapsed_time(f1) / e2e_steps
     if extras:
-        (graph_ms, fused_ms, fused_kernel_ms, hits_fused, ms_e2e, hits_e2e, e2e_steps, ms_pipe, hits_pipe, pipe_steps) = \
+        (graph_ms, fused_ms, fused_kernel_ms, hits_fused, ms_e2e, hits_e2e, e2e_steps, ms_pipe, hits_pipe, pipe_steps, d2h_pipe) = \
             extra_legs(torch, P, args, dev, step, barrier, d_x, h_x, st, ws, out, cnt, arena, n_dm, n_t, nmax, nmax_sigma, mode, thr, cap)
     del arena
     dec = None
@@ -510,7 +511,7 @@ def run_ours(args):
                            ("spd_search_host (pinned host buffers; H2D, spd_stats, spd_search_fused, D2H of statistics, count and records; "
                             "the SNR / width planes are never written on this path)")},
             "e2e_pipelined": {"value": nan_to_none(n / (ms_pipe * 1e-3)), "unit": "samples/s per GPU", "ms_per_step": nan_to_none(ms_pipe), "steps": pipe_steps,
-                              "hits": hits_pipe, "h2d_bytes_per_step": n * 4, "d2h_bytes_per_step": 8 + P.STATS_DTYPE.itemsize + 16 * cap,
+                              "hits": hits_pipe, "h2d_bytes_per_step": n * 4, "d2h_bytes_per_step": d2h_pipe,
                               "api": "paper_1611_09704_b200.stream.ChunkStream (two slots: H2D of chunk i+1 overlaps spd_stats + spd_search_fused of chunk i)"},
             "gpu_launches": launches_per_step * args.steps,
             "roofline": roof,

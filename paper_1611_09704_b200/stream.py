@@ -2,8 +2,12 @@
 
 A telescope back-end produces one de-dispersed chunk [n_dm][n_t] after another.  `ChunkStream` keeps `depth` device
 slots; the host-to-device copy of chunk i+1 runs on a copy stream while spd_stats + spd_search_fused (or, on request,
-spd_search_fused_decimated) of chunk i run on a compute stream, and the statistics, the hit count and the records of a finished chunk come back through pinned host
-buffers.  This module is plumbing only (CUDA streams and events from PyTorch, argument marshalling); every step of
+spd_search_fused_decimated) of chunk i run on a compute stream, and the statistics, the hit count and the records of a
+finished chunk come back through pinned host buffers: the count, the statistics and the first SPEC_RECORDS records (64 KiB)
+right behind the search, the rest of the list, if there is more, in one count-sized copy when the result is collected.
+Only a contiguous pinned chunk is copied straight from where it lies; any other source (a time slice of a longer pinned
+series, pageable memory) first goes through the slot's own pinned staging buffer, one host memcpy, so that the
+host-to-device copy stays asynchronous and keeps overlapping the previous chunk's search.  This module is plumbing only (CUDA streams and events from PyTorch, argument marshalling); every step of
 the search runs in the kernels behind the C ABI.
 
 Chunks along TIME for the same DM trials must overlap by Nmax - 1 samples: the last Nmax - 1 samples of a row see only
@@ -43,6 +47,9 @@ def time_chunks(n_total: int, chunk_len: int, nmax: int, align: int = 1) -> List
         s += step
 
 
+SPEC_RECORDS = 4096      # records copied back with the count, before the host knows how many there are (64 KiB)
+
+
 class ChunkStream:
     def __init__(self, n_dm: int, n_t: int, nmax: int, mode="sqrt", threshold: float = 6.0, capacity: int = 1 << 20,
                  depth: int = 2, device="cuda", decimated: Optional[Tuple[int, int]] = None):
@@ -61,6 +68,7 @@ class ChunkStream:
         self.dev = torch.device(device)
         self.copy_stream = torch.cuda.Stream(self.dev)
         self.compute_stream = torch.cuda.Stream(self.dev)
+        self.fetch_stream = torch.cuda.Stream(self.dev)       # remainder of a long list: must not queue behind the next chunk's search
         self.nsig = self.nmax if B._MODES[mode] != 0 else 0
         self.slots = []
         for _ in range(depth):
@@ -74,15 +82,20 @@ class ChunkStream:
                 "h_out": torch.zeros((self.capacity, 4), dtype=torch.int32).pin_memory(),
                 "h_cnt": torch.zeros(1, dtype=torch.int64).pin_memory(),
                 "h_stats": torch.zeros(B.STATS_BYTES, dtype=torch.uint8).pin_memory(),
+                "h_x": None,                                       # pinned staging buffer, made on first need
                 "copied": torch.cuda.Event(), "done": torch.cuda.Event(), "busy": False,
             })
         self.next_slot = 0
         self.bytes_h2d = n_dm * n_t * 4
+        self.spec = min(self.capacity, SPEC_RECORDS)
+        self.bytes_d2h = 0                                     # device-to-host bytes moved for the chunk collected last
 
     def submit(self, h_x: torch.Tensor, stats: Optional[torch.Tensor] = None) -> int:
-        """Enqueue one chunk (a pinned CPU float32 [n_dm][n_t] tensor, unit time stride, makes the copy asynchronous);
-        returns a ticket.  The slot's previous result must have been collected.  `stats`: a device spd_stats_t to search
-        with (e.g. the statistics of a longer stretch of data) instead of measuring them on this chunk."""
+        """Enqueue one chunk (a CPU float32 [n_dm][n_t] tensor with unit time stride); returns a ticket.  A contiguous
+        pinned tensor is copied asynchronously as it is; a row-strided or pageable one is first copied (on the host, now)
+        into the slot's pinned staging buffer.  The slot's previous result must have been collected.  `stats`: a device
+        spd_stats_t to search with (e.g. the statistics of a longer stretch of data) instead of measuring them on this
+        chunk."""
         if h_x.is_cuda or h_x.dtype != torch.float32 or tuple(h_x.shape) != (self.n_dm, self.n_t) or h_x.stride(1) != 1:
             raise B.SpdError("h_x must be a CPU float32 [n_dm][n_t] tensor of the stream's shape with unit time stride")
         k = self.next_slot
@@ -90,6 +103,13 @@ class ChunkStream:
         if s["busy"]:
             raise B.SpdError("ChunkStream: collect the result of the oldest chunk before submitting another")
         self.next_slot = (k + 1) % len(self.slots)
+        if not (h_x.is_contiguous() and h_x.is_pinned()):
+            # torch would gather a strided source into a pageable temporary and copy that synchronously; the slot is free
+            # (its last result was collected), so its staging buffer is no longer being read by an earlier copy
+            if s["h_x"] is None:
+                s["h_x"] = torch.empty((self.n_dm, self.n_t), dtype=torch.float32).pin_memory()
+            s["h_x"].copy_(h_x)
+            h_x = s["h_x"]
         with torch.cuda.stream(self.copy_stream):
             s["x"].copy_(h_x, non_blocking=True)
             s["copied"].record(self.copy_stream)
@@ -107,7 +127,7 @@ class ChunkStream:
                                              s["out"], s["cnt"], ws=s["dws"], stream=self.compute_stream)
             s["h_cnt"].copy_(s["cnt"], non_blocking=True)
             s["h_stats"].copy_(s["stats"], non_blocking=True)
-            s["h_out"].copy_(s["out"], non_blocking=True)          # whole buffer: the count is not known on the host yet
+            s["h_out"][:self.spec].copy_(s["out"][:self.spec], non_blocking=True)   # the count is not known on the host yet
             s["done"].record(self.compute_stream)
         s["busy"] = True
         return k
@@ -122,6 +142,12 @@ class ChunkStream:
         s["busy"] = False
         total = B.check_count(int(s["h_cnt"][0]))      # raises on the 'sigma_N undefined' sentinel (stats of another Nmax)
         got = min(total, self.capacity)
+        self.bytes_d2h = 8 + B.STATS_BYTES + 16 * self.spec
+        if got > self.spec:                                    # a long list: the remainder in one copy of exactly its size
+            with torch.cuda.stream(self.fetch_stream):         # the chunk is done (event above), so no ordering is needed
+                s["h_out"][self.spec:got].copy_(s["out"][self.spec:got], non_blocking=True)
+            self.fetch_stream.synchronize()
+            self.bytes_d2h += 16 * (got - self.spec)
         rec = s["h_out"][:got].numpy().view(B.CAND_DTYPE).reshape(-1)
         return rec, total, s["h_stats"].numpy().view(B.STATS_DTYPE)
 

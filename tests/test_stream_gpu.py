@@ -171,3 +171,33 @@ def test_time_axis_chunks_of_a_decimated_stream_equal_the_oracle_on_the_whole_se
                                          x, st.mean, o["sig"])
     assert r and total > 50, str(r)
     assert (rec["t"] >= T - 20).any() and (rec["width"] > w0).any()
+
+
+def test_chunk_stream_strided_and_pageable_sources_and_long_lists(P):
+    """A time slice of a longer pinned series (row-strided) and a pageable tensor go through the slot's pinned staging buffer;
+    a list longer than the SPEC_RECORDS copied with the count comes back whole through the count-sized second copy.  All
+    three must give the records of the contiguous pinned chunk, byte for byte, and bytes_d2h must be what was moved."""
+    from paper_1611_09704_b200 import stream as S
+    n_dm, n_t, nmax, cap = 8, 8192, 16, 1 << 15
+    rng = np.random.Generator(np.random.PCG64(4242))
+    series = torch.from_numpy(rng.standard_normal((n_dm, 3 * n_t)).astype(np.float32)).pin_memory()
+    view = series[:, n_t // 2:n_t // 2 + n_t]
+    assert not view.is_contiguous()
+    srcs = {"pinned": view.contiguous().pin_memory(), "strided": view, "pageable": view.contiguous()}
+    assert srcs["pinned"].is_pinned() and not srcs["pageable"].is_pinned()
+    for thr, long_list in ((4.5, False), (1.5, True)):
+        got = {}
+        for name, h in srcs.items():
+            cs = S.ChunkStream(n_dm, n_t, nmax, "sqrt", thr, capacity=cap, depth=2)
+            res = cs.run([h, h, h])                            # slot reuse: the staging buffer is rewritten while the pipeline runs
+            assert all(r[1] == res[0][1] for r in res)
+            rec, total = res[-1]
+            assert total <= cap and rec.size == total
+            assert (total > S.SPEC_RECORDS) == long_list
+            assert cs.bytes_d2h == 8 + P.STATS_DTYPE.itemsize + 16 * max(total, S.SPEC_RECORDS)
+            got[name] = np.sort(rec, order=["dm", "t"]).tobytes()
+        d = srcs["pinned"].cuda()
+        out, cnt = P.spd_search_fused(d, P.spd_stats(d), nmax, "sqrt", thr, capacity=cap)
+        want, total = P.read_candidates(out, cnt)
+        assert got["pinned"] == np.sort(want, order=["dm", "t"]).tobytes()
+        assert got["strided"] == got["pinned"] and got["pageable"] == got["pinned"]
