@@ -160,10 +160,14 @@ spd_status spd_stats_rows_noalloc(const float *d_x, int64_t n_dm, int64_t n_t, i
  * decimation in time of the input data"; the paper names the route, the algorithm is reading A20 of DESIGN.md).
  * An APPROXIMATION of spd_boxcar_snr with nmax = w0 * 2^(levels-1): the width grid gets coarser with width
  * (PAPER.md:21, :69 warn about the sensitivity this costs: at most 1 - sqrt(0.9) = 5.1 % for w0 = 16).
- *   level 0: every width 1..w0 at every sample (exactly spd_boxcar_snr with nmax = w0);
+ *   level 0: every width 1..w0 at every sample (exactly spd_boxcar_snr with nmax = w0 in the SQRT mode; in the LINEAR
+ *            modes sigma_N is that of the whole search, Nmax = w0 * 2^(levels-1), so it equals the widths 1..w0 of
+ *            spd_boxcar_snr with nmax = Nmax);
  *   level l: x_l[i] = x_{l-1}[2i] + x_{l-1}[2i+1] (n_l = n_t >> l samples per row), widths w' = w0/2+1..w0 of x_l at every
  *            decimated sample i: effective width N = w' 2^l, start sample t = i 2^l,
  *            SNR = (B - N mu) / sigma_N with sigma_N of the exhaustive search of the same nmax (eq. 4 / eq. 5 / anchored).
+ * The kernels form the level series from the mean-subtracted samples (x_1[i] = (x[2i] - mu) + (x[2i+1] - mu), in fp32), so a
+ * baseline far above the noise (|mu| = 1e3 sigma and more) costs the higher levels no precision.
  * Planes are packed per row: level l occupies elements [spd_decimated_level_offset(n_t, l), + n_l) of a row of
  * plane_stride elements (>= spd_decimated_level_offset(n_t, levels), a multiple of 8).  d_width holds the EFFECTIVE width
  * N; a position where none of the level's widths fits has snr = -inf, width = 0.
@@ -202,7 +206,9 @@ size_t spd_search_host_arena_bytes(int64_t n_dm, int64_t n_t, int nmax, uint64_t
  * spd_search_fused (the list is the product; the planes are not materialised), and copies the
  * statistics, the hit count and the first min(count, capacity) records back.  h_x / h_out / h_count /
  * h_stats are HOST pointers (pinned memory makes the copies asynchronous); d_arena is a caller-owned DEVICE
- * buffer of >= spd_search_host_arena_bytes(), 256-byte aligned.  This call SYNCHRONISES `stream` before it returns. */
+ * buffer of >= spd_search_host_arena_bytes(), 256-byte aligned.  This call SYNCHRONISES `stream` before it returns
+ * (once when count <= 4096: the first min(capacity, 4096) slots of h_out are copied together with the count, so h_out
+ * entries past the count, up to that many, hold unspecified bytes afterwards; a longer list takes a second copy). */
 spd_status spd_search_host(const float *h_x, int64_t n_dm, int64_t n_t, int nmax, spd_sigma_mode mode,
                            float threshold, spd_candidate_t *h_out, uint64_t capacity,
                            unsigned long long *h_count, spd_stats_t *h_stats,

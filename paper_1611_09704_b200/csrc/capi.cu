@@ -330,10 +330,13 @@ spd_status spd_search_host(const float *h_x, int64_t n_dm, int64_t n_t, int nmax
     if (st != SPD_OK) return st;
     if (h_stats && cudaMemcpyAsync(h_stats, d_stats, sizeof(spd_stats_t), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
     if (cudaMemcpyAsync(h_count, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
+    // the first records travel with the count (64 KiB at most), so a short list costs one synchronisation, not two
+    const unsigned long long spec = capacity < 4096 ? capacity : 4096;
+    if (spec > 0 && cudaMemcpyAsync(h_out, d_out, (size_t)spec * sizeof(spd_candidate_t), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
     if (cudaStreamSynchronize(s) != cudaSuccess) return SPD_ERR_CUDA;
-    const unsigned long long got = *h_count < capacity ? *h_count : capacity;
-    if (got > 0) {
-        if (cudaMemcpyAsync(h_out, d_out, (size_t)got * sizeof(spd_candidate_t), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
+    const unsigned long long got = *h_count < capacity ? *h_count : capacity;     // (UINT64_MAX, the sigma_N sentinel, has written no record)
+    if (*h_count != ~0ULL && got > spec) {
+        if (cudaMemcpyAsync(h_out + spec, d_out + spec, (size_t)(got - spec) * sizeof(spd_candidate_t), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
         if (cudaStreamSynchronize(s) != cudaSuccess) return SPD_ERR_CUDA;
     }
     return SPD_OK;
