@@ -152,6 +152,36 @@ def test_sweep_integer_data_forced_stats(P, n_dm, n_t, nmax):
     _sweep_case(P, x, nmax, "sqrt", UNIT)
 
 
+@pytest.mark.parametrize("nmax", [16, 20, 24, 32, 64, 128])
+def test_exact_ties_of_a_negative_maximum(P, nmax):
+    """What include/spd.h and DESIGN.md section 5 promise about EXACT ties, on integer data where every SNR involved is exact
+    in fp32 (r_1 = 1, r_4 = 1/2, r_16 = 1/4): the SNR plane holds the maximum itself; a non-negative maximum reports the
+    smallest tied width (reading A7); a NEGATIVE maximum reports one of the tied widths (the mantissa tags order the wrong
+    way below zero); the fused search replays a hit's sums and reports the smallest width in every case."""
+    from gpu_util import gpu_sweep, to_dev, gpu_fused
+    n_t = 1200
+    x = np.full((2, n_t), -8.0, dtype=np.float32)
+    x[0, 100:104] = [-2, -1, -1, 0]                        # widths 1 and 4 tie at -2 (2: -2.12, 3: -2.31, wider: below -5)
+    x[0, 300:316] = [-2, -3, -3] + [0] * 13                # widths 1 and 16 tie at -2 (two different 8-blocks of the general kernel)
+    x[1, 500:504] = [2, -1, 0, 3]                          # widths 1 and 4 tie at +2
+    sig = O.sigma_table(1.0, 0.0, nmax, "sqrt")
+    o_snr, o_w, o_m = O.sweep(x, 0.0, sig)
+    assert o_snr[0, 100] == -2.0 and o_w[0, 100] == 1 and o_m[0, 100] == 0.0     # the oracle: smallest width, margin 0
+    assert o_snr[0, 300] == -2.0 and o_w[0, 300] == 1 and o_m[0, 300] == 0.0
+    assert o_snr[1, 500] == 2.0 and o_w[1, 500] == 1 and o_m[1, 500] == 0.0
+    st = P.write_stats(0.0, 1.0)
+    g_snr, g_w, _ = gpu_sweep(x, st, nmax, "sqrt")
+    assert CMP.compare_planes(x, 0.0, sig, g_snr, g_w, o_snr, o_w, o_m)
+    assert g_snr[0, 100] == -2.0 and g_snr[0, 300] == -2.0 and g_snr[1, 500] == 2.0
+    assert g_w[1, 500] == 1                                # non-negative maximum: the smallest width, exactly
+    assert g_w[0, 100] in (1, 4) and g_w[0, 300] in (1, 16)
+    rec, total = gpu_fused(to_dev(x), st, nmax, "sqrt", -2.5)
+    hits = {(int(r["dm"]), int(r["t"])): r for r in rec}
+    assert total == len(hits) and {(0, 100), (0, 300), (1, 500)} <= set(hits)
+    for key, snr in (((0, 100), -2.0), ((0, 300), -2.0), ((1, 500), 2.0)):
+        assert hits[key]["snr"] == np.float32(snr) and hits[key]["width"] == 1, (key, hits[key])
+
+
 @pytest.mark.parametrize("n_dm,n_t,nmax,mu,sigma", [
     (4, 4096, 32, 0.0, 1.0), (3, 6000, 128, 0.0, 1.0), (3, 5000, 64, 100.0, 20.0), (2, 7777, 512, 0.0, 1.0),
     (2, 4100, 100, -1000.0, 1.0), (64, 2048, 8, 0.0, 1.0),
