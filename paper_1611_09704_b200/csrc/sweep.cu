@@ -154,10 +154,12 @@ cudaError_t launch_sigma_table(const spd_stats_t *d_stats, int nmax, int mode, f
 // ---- decimation in time (reading A20): x_l[i] = x_{l-1}[2i] + x_{l-1}[2i+1]; the statistics of a level are those
 // of x scaled to sums of D = 2^l samples: mean_l = D mu, sigma_l = sqrt(D) sigma (eq. 3), so that eq. 4 of the decimated
 // series at width w' IS eq. 4 of x at the effective width w' D.  Nothing is re-measured.
+// The level kernels carry the series with the mean already taken out (level 0 subtracts mu from every sample before it
+// forms the pair sums, Norm::apply_pair_sum), so above level 0 the mean handed to the kernel is 0, not D mu.
 __global__ void level_stats_kernel(const spd_stats_t *__restrict__ st, int D, spd_stats_t *__restrict__ out)
 {
     spd_stats_t s = *st;
-    s.mean = st->mean * (double)D;
+    s.mean = D == 1 ? st->mean : 0.0;
     s.sigma = st->sigma * sqrt((double)D);
     *out = s;
 }
@@ -285,6 +287,22 @@ struct Norm {
             op = __fadd_rn(v.x, mu_lo2.x); oq = __fadd_rn(v.y, mu_lo2.x);
         }
     }
+    // apply_pair, and sum = y_p + y_q of the mean-subtracted samples BEFORE the 1/sigma scaling: one sample of the next
+    // decimated level.  Summing y instead of the raw x keeps the level series at the size of the noise, not of D mu
+    // (a baseline of 1e3 sigma would otherwise cost ulp(D mu) per level in every SNR above level 0).
+    template <bool RC>
+    __device__ __forceinline__ void apply_pair_sum(float p, float q, float &op, float &oq, float &sum) const
+    {
+        float2 v = __fadd2_rn(make_float2(p, q), mu_hi2);
+        if (RC) {
+            v = __fadd2_rn(v, mu_lo2);
+            sum = __fadd_rn(v.x, v.y);
+            op = __fmul_rn(v.x, rs2.x); oq = __fmul_rn(v.y, rs2.x);
+        } else {
+            op = __fadd_rn(v.x, mu_lo2.x); oq = __fadd_rn(v.y, mu_lo2.x);
+            sum = __fadd_rn(op, oq);
+        }
+    }
 };
 
 // 8 groups of one raw tile -> 8 interleaved values (sub-tile A, sub-tile B) of group g
@@ -303,9 +321,12 @@ __device__ __forceinline__ void load_norm_group(const float *raw, int g, const N
 {
     const float4 a0 = *reinterpret_cast<const float4 *>(raw + 8 * g), a1 = *reinterpret_cast<const float4 *>(raw + 8 * g + 4);
     const float4 b0 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g), b1 = *reinterpret_cast<const float4 *>(raw + SW_SUB + 8 * g + 4);
-    if (PAIRSUMS) {                                   // x'[i] = x[2i] + x[2i+1] of the RAW samples (decimation in time)
-        *sa = make_float4(__fadd_rn(a0.x, a0.y), __fadd_rn(a0.z, a0.w), __fadd_rn(a1.x, a1.y), __fadd_rn(a1.z, a1.w));
-        *sb = make_float4(__fadd_rn(b0.x, b0.y), __fadd_rn(b0.z, b0.w), __fadd_rn(b1.x, b1.y), __fadd_rn(b1.z, b1.w));
+    if (PAIRSUMS) {                                   // x'[i] = y[2i] + y[2i+1], y = x - mu (decimation in time; the level's mean is then 0)
+        norm.apply_pair_sum<RC>(a0.x, a0.y, v[0].x, v[1].x, sa->x); norm.apply_pair_sum<RC>(a0.z, a0.w, v[2].x, v[3].x, sa->y);
+        norm.apply_pair_sum<RC>(a1.x, a1.y, v[4].x, v[5].x, sa->z); norm.apply_pair_sum<RC>(a1.z, a1.w, v[6].x, v[7].x, sa->w);
+        norm.apply_pair_sum<RC>(b0.x, b0.y, v[0].y, v[1].y, sb->x); norm.apply_pair_sum<RC>(b0.z, b0.w, v[2].y, v[3].y, sb->y);
+        norm.apply_pair_sum<RC>(b1.x, b1.y, v[4].y, v[5].y, sb->z); norm.apply_pair_sum<RC>(b1.z, b1.w, v[6].y, v[7].y, sb->w);
+        return;
     }
     norm.apply_pair<RC>(a0.x, a0.y, v[0].x, v[1].x); norm.apply_pair<RC>(a0.z, a0.w, v[2].x, v[3].x);
     norm.apply_pair<RC>(a1.x, a1.y, v[4].x, v[5].x); norm.apply_pair<RC>(a1.z, a1.w, v[6].x, v[7].x);

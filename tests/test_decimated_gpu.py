@@ -266,3 +266,16 @@ def test_fused_decimated_search_is_cuda_graph_capturable(P):
     assert int(cnt.item()) == n0 > 0
     got = np.sort(out[:n0].cpu().numpy().view(P.CAND_DTYPE).reshape(-1), order=["dm", "t", "width"])
     assert got.tobytes() == ref.tobytes()
+
+
+@pytest.mark.parametrize("mode", ["sqrt", "anchored"])
+@pytest.mark.parametrize("mu,sigma", [(-1000.0, 1.0), (10000.0, 1.0), (3.0e5, 100.0)])
+def test_decimated_baseline_far_above_the_noise(P, mode, mu, sigma):
+    """|mu| = 1e3 .. 1e4 sigma through all 8 levels (Nmax 2048), planes and fused search: the level series are built from the
+    mean-subtracted samples, so the SNR of the high levels must not pick up the rounding of D mu (ulp(256 * 1e4) = 0.25)."""
+    x = (mu + sigma * rng(650).standard_normal((2, 20001))).astype(np.float32)
+    x[1, 6000:7200] += np.float32(0.3 * sigma)              # a wide pulse for the top levels
+    lv, infos = _run(P, x, 16, 8, mode, thr=5.0)
+    assert lv[-1]["level"] == 7 and (lv[-1]["snr"] >= 5.0).any()
+    rec, info = _run_fused(P, x, 16, 8, mode, thr=5.0)
+    assert info["gpu_hits"] > 0 and (rec["width"] > 1024).any()
