@@ -1,7 +1,6 @@
 """Builds libspd.so (the C-ABI library of include/spd.h) in-tree with nvcc for sm_100a.
 
     python -m paper_1611_09704_b200.build [--force] [--verbose]
-    python -m paper_1611_09704_b200.build --ubench      (csrc/ubench_fp32.cu -> ./ubench_fp32, the issue-rate microbenchmark)
 """
 from __future__ import annotations
 
@@ -42,14 +41,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_ubench() -> str:
-    """The fp32 issue-rate microbenchmark behind the sweep's ALU roofline (csrc/ubench_fp32.cu): a stand-alone program."""
-    exe = os.path.join(HERE, "ubench_fp32")
-    subprocess.check_call([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-                           "-o", exe, os.path.join(CSRC, "ubench_fp32.cu")])
-    return exe
-
-
 def ensure_built() -> str:
     """Build libspd.so if it is not there at all (a fresh clone: built artefacts are git-ignored).  Callers that time
     or test the library use this; the library itself never builds or falls back (binding.lib() raises)."""
@@ -57,7 +48,4 @@ def ensure_built() -> str:
 
 
 if __name__ == "__main__":
-    if "--ubench" in sys.argv:
-        print(build_ubench())
-    else:
-        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

@@ -7,7 +7,7 @@
 // (planes, nmax <= 32; also one level of the decimated search), boxcar_search_fused (threshold in the kernel, no planes) and
 // boxcar_search_fused_level (the same for one level of the decimated search).
 //
-// What bounds the loop (measured with csrc/ubench_fp32.cu, profiles/r02_fp32_issue_rates.md): one warp instruction per
+// What bounds the loop (measured with a microbenchmark, profiles/r02_fp32_issue_rates.md): one warp instruction per
 // sub-partition per clock, a packed FADD2 / FMUL2 counts as two (it passes the 32-lane FMA pipe twice), an ALU-pipe
 // instruction (FMNMX3, LOP3, FSETP, SEL) occupies its 16-lane pipe for two clocks.  One (sample, width) pair needs an add,
 // a multiply and half a 3-input maximum = 2.5 issue slots; everything else in this file exists to add as little as
