@@ -84,6 +84,49 @@ def test_stats_with_one_huge_outlier(P, where, nmax):
     assert r, str(r)
 
 
+def _check_global_stats(P, x, nmax):
+    from gpu_util import gpu_stats
+    g, _ = gpu_stats(x, nmax)
+    o = O.full_stats(x, nmax)
+    r = CMP.compare_stats(float(g["mean"]), float(g["sigma"]), o, float(g["sigma_nmax"]))
+    assert r, f"nmax {nmax}: {r}"
+
+
+@pytest.mark.parametrize("nmax", [16, 512, 4096])
+def test_global_stats_of_rows_with_very_different_baselines(P, nmax):
+    """The GLOBAL spd_stats (one estimate over everything, reading A3) on rows whose means differ by 1e3 of their own sigma: a
+    persistent CTA walks tiles of many rows, so whatever it shifts the data by must not be tied to the first tile it sees."""
+    r = rng(105)
+    n_dm, n_t = 24, 3 * 4096 + 1000
+    mu = r.uniform(-1000.0, 1000.0, n_dm)
+    x = (mu[:, None] + r.standard_normal((n_dm, n_t))).astype(np.float32)
+    _check_global_stats(P, x, nmax)
+
+
+@pytest.mark.parametrize("nmax", [512, 4096])
+@pytest.mark.parametrize("n_dm,n_t", [(8, 5 * 4096), (300, 2 * 4096 + 100)])
+def test_global_stats_with_a_baseline_excursion_on_the_first_tile(P, nmax, n_dm, n_t):
+    """One 4096-sample stretch 300 sigma above everything else (a saturated RFI burst) exactly where persistent CTAs start
+    their walk: tile 0 of row 0, and the tiles later CTAs start on.  sigma_Nmax must still come out to 1e-6."""
+    r = rng(106)
+    x = (5.0 + r.standard_normal((n_dm, n_t))).astype(np.float32)
+    x[0, :4096] += 300.0
+    x[n_dm // 2, 4096:8192] += 300.0
+    x[n_dm - 1, :4096] += 300.0
+    _check_global_stats(P, x, nmax)
+
+
+@pytest.mark.parametrize("nmax", [64, 1024])
+def test_global_stats_with_a_drifting_baseline(P, nmax):
+    """Config-4-like slow baseline drift, 50 sigma peak to peak over each row, with a different phase per row."""
+    r = rng(107)
+    n_dm, n_t = 16, 40000
+    t = np.arange(n_t)[None, :] / n_t
+    ph = r.uniform(0, 2 * np.pi, n_dm)[:, None]
+    x = (25.0 * np.sin(2 * np.pi * 1.5 * t + ph) + r.standard_normal((n_dm, n_t))).astype(np.float32)
+    _check_global_stats(P, x, nmax)
+
+
 def test_stats_is_bit_reproducible(P):
     from gpu_util import gpu_stats
     x = (100 + 20 * rng(102).standard_normal((64, 16384))).astype(np.float32)
