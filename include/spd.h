@@ -214,6 +214,17 @@ spd_status spd_search_host(const float *h_x, int64_t n_dm, int64_t n_t, int nmax
                            unsigned long long *h_count, spd_stats_t *h_stats,
                            void *d_arena, size_t arena_bytes, void *stream);
 
+/* spd_search_host with the decimated search (the real-time route for wide filters): copies h_x to the device,
+ * runs spd_stats (with sigma_Nmax of Nmax = w0 * 2^(levels-1) in the LINEAR modes) and spd_search_fused_decimated, and copies
+ * the statistics, the hit count and the records back.  Arguments, the h_out convention and the synchronisation follow
+ * spd_search_host; w0 / levels follow spd_boxcar_snr_decimated; d_arena: >= spd_search_host_decimated_arena_bytes() bytes
+ * (0 = invalid arguments), 256-byte aligned. */
+size_t spd_search_host_decimated_arena_bytes(int64_t n_dm, int64_t n_t, int w0, int levels, uint64_t capacity);
+spd_status spd_search_host_decimated(const float *h_x, int64_t n_dm, int64_t n_t, int w0, int levels, spd_sigma_mode mode,
+                                     float threshold, spd_candidate_t *h_out, uint64_t capacity,
+                                     unsigned long long *h_count, spd_stats_t *h_stats,
+                                     void *d_arena, size_t arena_bytes, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -52,6 +52,8 @@ def lib() -> C.CDLL:
         L.spd_search_fused.argtypes = [vp, i64, i64, i64, vp, i32, i32, f32, vp, u64, vp, vp, sz, vp]
         L.spd_search_host_arena_bytes.argtypes = [i64, i64, i32, u64]; L.spd_search_host_arena_bytes.restype = sz
         L.spd_search_host.argtypes = [vp, i64, i64, i32, i32, f32, vp, u64, vp, vp, vp, sz, vp]
+        L.spd_search_host_decimated_arena_bytes.argtypes = [i64, i64, i32, i32, u64]; L.spd_search_host_decimated_arena_bytes.restype = sz
+        L.spd_search_host_decimated.argtypes = [vp, i64, i64, i32, i32, i32, f32, vp, u64, vp, vp, vp, sz, vp]
         L.spd_workspace_bytes_rows.argtypes = [i64, i64, i32]; L.spd_workspace_bytes_rows.restype = sz
         L.spd_stats_rows.argtypes = [vp, i64, i64, i64, i32, vp, vp, sz, vp]
         L.spd_stats_rows_noalloc.argtypes = [vp, i64, i64, i64, i32, vp, vp]
@@ -65,7 +67,7 @@ def lib() -> C.CDLL:
         L.spd_search_fused_decimated.argtypes = [vp, i64, i64, i64, vp, i32, i32, i32, f32, vp, u64, vp, vp, sz, vp]
         for f in ("spd_stats", "spd_stats_merge", "spd_boxcar_snr", "spd_candidates", "spd_search_fused", "spd_search_host",
                   "spd_boxcar_snr_decimated", "spd_candidates_decimated", "spd_search_fused_decimated", "spd_stats_rows", "spd_boxcar_snr_rows",
-                  "spd_search_fused_rows", "spd_stats_rows_noalloc"):
+                  "spd_search_fused_rows", "spd_stats_rows_noalloc", "spd_search_host_decimated"):
             getattr(L, f).restype = i32
         _lib = L
     return _lib
@@ -331,4 +333,23 @@ def spd_search_host(h_x: torch.Tensor, nmax: int, mode, threshold: float, h_out:
     _check(lib().spd_search_host(h_x.data_ptr(), n_dm, n_t, int(nmax), _MODES[mode], float(threshold), h_out.data_ptr(),
                                  h_out.shape[0], h_count.data_ptr(), h_stats.data_ptr() if h_stats is not None else None,
                                  arena.data_ptr(), arena.numel(), _stream(stream)), "spd_search_host")
-    return int(h_count[0])
+    return check_count(int(h_count[0]))
+
+
+def search_host_decimated_arena_bytes(n_dm: int, n_t: int, w0: int, levels: int, capacity: int) -> int:
+    return int(lib().spd_search_host_decimated_arena_bytes(n_dm, n_t, w0, levels, capacity))
+
+
+def spd_search_host_decimated(h_x: torch.Tensor, w0: int, levels: int, mode, threshold: float, h_out: torch.Tensor,
+                              h_count: torch.Tensor, h_stats: Optional[torch.Tensor], arena: torch.Tensor, stream=None) -> int:
+    """spd_search_host with the decimated search (Nmax = w0 * 2^(levels-1)); returns the hit count.  Synchronises."""
+    if h_x.is_cuda or h_x.dtype != torch.float32 or h_x.dim() != 2 or not h_x.is_contiguous():
+        raise SpdError("h_x must be a contiguous CPU float32 [n_dm][n_t] tensor")
+    if h_out.is_cuda or h_out.dtype != torch.int32 or h_out.dim() != 2 or h_out.shape[1] != 4 or h_count.is_cuda:
+        raise SpdError("h_out must be a CPU int32 [capacity][4] tensor, h_count a CPU int64 tensor")
+    n_dm, n_t = h_x.shape
+    _check(lib().spd_search_host_decimated(h_x.data_ptr(), n_dm, n_t, int(w0), int(levels), _MODES[mode], float(threshold),
+                                           h_out.data_ptr(), h_out.shape[0], h_count.data_ptr(),
+                                           h_stats.data_ptr() if h_stats is not None else None,
+                                           arena.data_ptr(), arena.numel(), _stream(stream)), "spd_search_host_decimated")
+    return check_count(int(h_count[0]))

@@ -342,4 +342,52 @@ spd_status spd_search_host(const float *h_x, int64_t n_dm, int64_t n_t, int nmax
     return SPD_OK;
 }
 
+// arena layout of spd_search_host_decimated: x | candidates | stats | count | workspace of the decimated search (which
+// covers the statistics' workspace: it starts with spd_workspace_bytes(.., w0) >= STATS_WS bytes)
+size_t spd_search_host_decimated_arena_bytes(int64_t n_dm, int64_t n_t, int w0, int levels, uint64_t capacity)
+{
+    const size_t ws = spd_decimated_workspace_bytes(n_dm, n_t, w0, levels);
+    if (ws == 0) return 0;
+    const size_t n = (size_t)n_dm * (size_t)n_t;
+    return align_up(n * 4, 256) + align_up((size_t)capacity * sizeof(spd_candidate_t), 256) + 256 + 256 + ws;
+}
+
+spd_status spd_search_host_decimated(const float *h_x, int64_t n_dm, int64_t n_t, int w0, int levels, spd_sigma_mode mode,
+                                     float threshold, spd_candidate_t *h_out, uint64_t capacity,
+                                     unsigned long long *h_count, spd_stats_t *h_stats,
+                                     void *d_arena, size_t arena_bytes, void *stream)
+{
+    if (!h_x || !h_count || (!h_out && capacity > 0) || !d_arena || !shape_ok(n_dm, n_t, n_t) || !dec_ok(w0, levels, n_t))
+        return SPD_ERR_INVALID_ARG;
+    if ((int)mode < 0 || (int)mode > 2 || (reinterpret_cast<uintptr_t>(d_arena) & 255) != 0) return SPD_ERR_INVALID_ARG;
+    if (arena_bytes < spd_search_host_decimated_arena_bytes(n_dm, n_t, w0, levels, capacity)) return SPD_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t n = (size_t)n_dm * (size_t)n_t;
+    unsigned char *p = reinterpret_cast<unsigned char *>(d_arena);
+    float *d_x = reinterpret_cast<float *>(p);                 p += align_up(n * 4, 256);
+    spd_candidate_t *d_out = reinterpret_cast<spd_candidate_t *>(p); p += align_up((size_t)capacity * sizeof(spd_candidate_t), 256);
+    spd_stats_t *d_stats = reinterpret_cast<spd_stats_t *>(p); p += 256;
+    unsigned long long *d_count = reinterpret_cast<unsigned long long *>(p); p += 256;
+    void *d_ws = p;
+    const size_t ws_bytes = spd_decimated_workspace_bytes(n_dm, n_t, w0, levels);
+    const int nmax_total = w0 << (levels - 1);
+
+    if (cudaMemcpyAsync(d_x, h_x, n * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPD_ERR_CUDA;
+    spd_status st = spd_stats(d_x, n_dm, n_t, n_t, mode == SPD_SIGMA_SQRT ? 0 : nmax_total, d_stats, d_ws, ws_bytes, stream);
+    if (st != SPD_OK) return st;
+    st = spd_search_fused_decimated(d_x, n_dm, n_t, n_t, d_stats, w0, levels, mode, threshold, d_out, capacity, d_count, d_ws, ws_bytes, stream);
+    if (st != SPD_OK) return st;
+    if (h_stats && cudaMemcpyAsync(h_stats, d_stats, sizeof(spd_stats_t), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
+    if (cudaMemcpyAsync(h_count, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
+    const unsigned long long spec = capacity < 4096 ? capacity : 4096;           // as spd_search_host: one synchronisation for a short list
+    if (spec > 0 && cudaMemcpyAsync(h_out, d_out, (size_t)spec * sizeof(spd_candidate_t), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
+    if (cudaStreamSynchronize(s) != cudaSuccess) return SPD_ERR_CUDA;
+    const unsigned long long got = *h_count < capacity ? *h_count : capacity;
+    if (*h_count != ~0ULL && got > spec) {
+        if (cudaMemcpyAsync(h_out + spec, d_out + spec, (size_t)(got - spec) * sizeof(spd_candidate_t), cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPD_ERR_CUDA;
+        if (cudaStreamSynchronize(s) != cudaSuccess) return SPD_ERR_CUDA;
+    }
+    return SPD_OK;
+}
+
 }  // extern "C"

@@ -114,3 +114,19 @@ def test_round2_entry_points_validate_arguments(L):
     assert L.spd_boxcar_snr_rows(fake, C.c_int64(4), C.c_int64(100), C.c_int64(100), fake, 40, 1, fake, fake, fake, C.c_size_t(64), None) == WS
     assert L.spd_search_fused_rows(fake, C.c_int64(4), C.c_int64(100), C.c_int64(100), fake, 40, 0, C.c_float(float("nan")), fake, C.c_uint64(4), fake,
                                    fake, C.c_size_t(1 << 20), None) == INV
+
+
+def test_search_host_decimated_validates_arguments(L):
+    fake = C.c_void_p(4096)
+    INV, WS = 1, 3
+    ab = L.spd_search_host_decimated_arena_bytes
+    assert ab(64, 16384, 16, 3, 1 << 12) >= 64 * 16384 * 4 + (16 << 12) + L.spd_decimated_workspace_bytes(C.c_int64(64), C.c_int64(16384), 16, 3)
+    assert ab(64, 16384, 24, 3, 1 << 12) == 0 and ab(64, 16384, 32, 9, 1 << 12) == 0 and ab(0, 16384, 16, 3, 16) == 0
+    f = L.spd_search_host_decimated
+    assert f(None, 2, 4096, 16, 2, 0, 6.0, fake, 10, fake, None, fake, 1 << 30, None) == INV
+    assert f(fake, 2, 4096, 16, 2, 0, 6.0, fake, 10, None, None, fake, 1 << 30, None) == INV
+    assert f(fake, 2, 4096, 16, 2, 0, 6.0, None, 10, fake, None, fake, 1 << 30, None) == INV
+    assert f(fake, 2, 4096, 24, 2, 0, 6.0, fake, 10, fake, None, fake, 1 << 30, None) == INV       # w0 must be 16 or 32
+    assert f(fake, 2, 4096, 16, 2, 5, 6.0, fake, 10, fake, None, fake, 1 << 30, None) == INV       # bad mode
+    assert f(fake, 2, 4096, 16, 2, 0, 6.0, fake, 10, fake, None, C.c_void_p(4097), 1 << 30, None) == INV   # arena alignment
+    assert f(fake, 2, 4096, 16, 2, 0, 6.0, fake, 10, fake, None, fake, 1024, None) == WS

@@ -5,11 +5,14 @@ Tolerances are BASELINE.json:north_star's, implemented in oracle/compare.py:
   near-ties (margin <= 1e-3); candidates equal as (dm, t) sets outside 1e-3 of the threshold.
 """
 import math
+import os
 
 import numpy as np
 import pytest
 
 import gen
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 from oracle import spd_oracle as O
 from oracle import compare as CMP
 
@@ -440,8 +443,11 @@ def test_config2_whole_path_every_row(P):
     assert info["rows"] == cfg.n_dm and info["samples"] == x.size
 
 
-def _survey_rows(cfg, cap_pulse_rows):
-    """every 16th row plus every pulse-bearing row and its +-3 neighbours, the latter capped."""
+def _survey_rows(cfg, cap_pulse_rows, full=False):
+    """every 16th row plus every pulse-bearing row and its +-3 neighbours, the latter capped; every row of
+    the array with --full."""
+    if full:
+        return list(range(cfg.n_dm))
     pulse = []
     for r in gen.pulse_rows(cfg):
         pulse += [q for q in range(r - 3, r + 4) if 0 <= q < cfg.n_dm]
@@ -458,22 +464,35 @@ def test_config3_whole_path_every_row(P):
     assert info["rows"] == cfg.n_dm and info["samples"] == x.size and total > 0
 
 
-def test_config4_eq5_whole_path_survey_rows(P):
+def _record_full(full, name, info):
+    """--full runs leave their counts (rows, samples, hits, exempted near-ties / near-threshold samples) in gpurun_out/."""
+    if full:
+        import json
+        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        with open(os.path.join(ROOT, "gpurun_out", "full_parity.jsonl"), "a") as f:
+            f.write(json.dumps({"case": name, **{k: (float(v) if isinstance(v, float) else int(v)) for k, v in info.items()}}) + "\n")
+
+
+def test_config4_eq5_whole_path_survey_rows(P, full_run):
     """BASELINE config 4 (signal-dominated, eq. 5 literal with the measured sigma_Nmax, Nmax 512): statistics on the full
     array; planes and candidates on every 16th row plus the pulse-bearing rows +-3 (capped at 192)."""
     cfg = gen.get_config(4)
     x = gen.make_array(cfg)
     # eq. 5 as printed flattens the SNR over the wide widths (sigma_N grows ~linearly), so near-ties are more frequent here (~5 %)
-    _whole_path(P, cfg, x, cfg.nmax[0], rows=_survey_rows(cfg, 192), tie_rate_max=0.10)
+    _, _, info = _whole_path(P, cfg, x, cfg.nmax[0], rows=_survey_rows(cfg, 192, full_run), tie_rate_max=0.10)
+    assert not full_run or info["rows"] == cfg.n_dm
+    _record_full(full_run, "config4 eq5 Nmax 512", info)
 
 
 @pytest.mark.parametrize("nmax", [8, 32, 128, 512])
-def test_config5_width_sweep_survey_rows(P, nmax):
+def test_config5_width_sweep_survey_rows(P, nmax, full_run):
     """BASELINE config 5 (4096 x 524288 = 2^31 samples: every flat offset must be 64-bit) at each Nmax of the sweep: every
     16th row plus pulse-bearing rows +-3 (capped at 64)."""
     cfg = gen.get_config(5)
     x = _c5_array(cfg)
-    _whole_path(P, cfg, x, nmax, rows=_survey_rows(cfg, 64), fused=(nmax == 32))
+    _, _, info = _whole_path(P, cfg, x, nmax, rows=_survey_rows(cfg, 64, full_run), fused=(nmax == 32 or full_run))
+    assert not full_run or info["rows"] == cfg.n_dm
+    _record_full(full_run, f"config5 Nmax {nmax}", info)
 
 
 _C5 = {}

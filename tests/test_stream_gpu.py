@@ -201,3 +201,32 @@ def test_chunk_stream_strided_and_pageable_sources_and_long_lists(P):
         want, total = P.read_candidates(out, cnt)
         assert got["pinned"] == np.sort(want, order=["dm", "t"]).tobytes()
         assert got["strided"] == got["pinned"] and got["pageable"] == got["pinned"]
+
+
+@pytest.mark.parametrize("mode,w0,levels,thr", [("sqrt", 16, 3, 6.0), ("linear", 16, 2, 4.0), ("sqrt", 32, 2, 2.5)])
+def test_search_host_decimated_equals_the_oracle(P, mode, w0, levels, thr):
+    """spd_search_host_decimated (host buffers in, host records out) against the ORACLE's decimated candidate list, and its
+    statistics against the oracle's; the last case has a list longer than the 4096 records that travel with the count."""
+    from oracle import spd_oracle as O
+    from oracle import compare as CMP
+    cfg = gen.get_config(1)
+    x = gen.make_array(cfg)
+    cap = 1 << 16
+    h_x = torch.from_numpy(x).pin_memory()
+    h_out = torch.zeros((cap, 4), dtype=torch.int32).pin_memory()
+    h_count = torch.zeros(1, dtype=torch.int64).pin_memory()
+    h_stats = torch.zeros(P.STATS_DTYPE.itemsize, dtype=torch.uint8).pin_memory()
+    arena = torch.empty(P.search_host_decimated_arena_bytes(cfg.n_dm, cfg.n_t, w0, levels, cap), dtype=torch.uint8, device="cuda")
+    total = P.spd_search_host_decimated(h_x, w0, levels, mode, thr, h_out, h_count, h_stats, arena)
+    rec = h_out[:min(total, cap)].numpy().view(P.CAND_DTYPE).reshape(-1)
+    o = O.search_decimated(x, w0, levels, mode, thr)
+    g = h_stats.numpy().view(P.STATS_DTYPE)[0]
+    r = CMP.compare_stats(float(g["mean"]), float(g["sigma"]), o["stats"], float(g["sigma_nmax"]) if mode != "sqrt" else None)
+    assert r, str(r)
+    r = CMP.compare_candidates_decimated(rec["dm"], rec["t"], rec["snr"], rec["width"], total, cap, o["levels"], w0, thr,
+                                         x, o["stats"].mean, o["sig"])
+    assert r and total > 0, str(r)
+    if thr < 3.0:
+        assert total > 4096
+    with pytest.raises(P.SpdError):
+        P.spd_search_host_decimated(h_x, w0, levels, mode, thr, h_out, h_count, h_stats, arena[:1024])
